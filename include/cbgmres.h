@@ -1,0 +1,167 @@
+/*
+ * cbgmres.h -- C ABI of the B200-native compressed-basis GMRES (CB-GMRES) hot path.
+ *
+ * Method: arXiv 2009.12101, "Compressed Basis GMRES on High Performance GPUs".  Citations are
+ * PAPER.md:<line> (the paper text) and the DESIGN.md reading they rely on.
+ *
+ * Problem statement: solve A x = b, A in R^{n x n} sparse with nnz nonzeros in
+ * CSR (fp64 values + 32-bit indices), by restarted GMRES (Fig. 1)
+ * with restart length m, classical Gram-Schmidt with optional re-orthogonalisation threshold eta
+ * (PAPER.md:104), stopping when ||b - A x||_2 <= tau ||b||_2.  The Krylov
+ * basis is kept in HBM in one of five storage formats while every arithmetic operation is IEEE
+ * binary64.
+ *
+ * Conventions
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  All buffers are owned by the
+ *     caller (torch tensors in the Python binding); the library only borrows them for the duration
+ *     of the call, except the CSR arrays given to cbgmres_set_matrix, which must stay valid until
+ *     the next set_matrix / destroy.
+ *   - Every call returns a cbgmres_status_t (0 = success).  No exceptions, no errno, no stdout.
+ *     On an invalid argument nothing is enqueued.  cbgmres_last_error gives a static string.
+ *   - The CUDA stream given to cbgmres_create is borrowed; every call enqueues on it.  Calls that
+ *     return results to the host (solve, solve_host) synchronise that stream before returning;
+ *     the k_* hooks and set_matrix only enqueue.
+ *   - Device memory: cbgmres_create allocates a fixed scratch block (reduction partials and the
+ *     solver's control block, a few MB); cbgmres_set_matrix may allocate O(nnz/1024) ints of
+ *     row-partition metadata.  cbgmres_solve allocates nothing: the basis and work vectors live in
+ *     the caller's workspace.
+ *   - One handle per host thread.  Basis offsets are 64-bit; CSR indices are 32-bit.
+ *   - A basis is stored vector-major: vector c occupies ld entries of the storage type starting
+ *     at entry c*ld; ld >= n and ld*bytes(format) must be a multiple of 16, base 16-byte aligned.
+ */
+#ifndef CBGMRES_H_
+#define CBGMRES_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cbgmres_ctx *cbgmres_handle_t;
+
+/* Storage formats of the basis: <float64>, <float32>, <float16> (IEEE casts,
+ * round-to-nearest-even, gradual underflow) and the fixed-point <int32>, <int16> with one scale
+ * sigma_j = ||v_j||inf / max_int per vector (readings Q6/Q7). */
+typedef enum {
+    CBGMRES_FP64 = 0,
+    CBGMRES_FP32 = 1,
+    CBGMRES_FP16 = 2,
+    CBGMRES_INT32 = 3,
+    CBGMRES_INT16 = 4
+} cbgmres_format_t;
+
+/* Fig. 1 lines 7-11: never, when h_{j+1,j} < eta*omega, or on every step. */
+typedef enum { CBGMRES_REORTH_NEVER = 0, CBGMRES_REORTH_COND = 1, CBGMRES_REORTH_ALWAYS = 2 } cbgmres_reorth_t;
+
+typedef enum {
+    CBGMRES_OK = 0,
+    CBGMRES_E_INVALID = 1,    /* bad argument (null pointer, n <= 0, restart < 1, unknown format ...) */
+    CBGMRES_E_NOMATRIX = 2,   /* solve / k_spmv before set_matrix */
+    CBGMRES_E_WORKSPACE = 3,  /* workspace too small or misaligned */
+    CBGMRES_E_CUDA = 4,       /* a CUDA runtime call failed; see cbgmres_last_error */
+    CBGMRES_E_NONFINITE = 5,  /* non-finite residual norm; x holds the last completed cycle */
+    CBGMRES_NOT_CONVERGED = 16 /* ran to max_iters; x is valid, result is filled */
+} cbgmres_status_t;
+
+#define CBGMRES_MAX_RESTART 512
+
+typedef struct {
+    int32_t restart;         /* m, 1..CBGMRES_MAX_RESTART (the paper uses 100, 10..300) */
+    int32_t max_iters;       /* bound on Arnoldi steps summed over all restart cycles */
+    int32_t format;          /* cbgmres_format_t */
+    int32_t reorth;          /* cbgmres_reorth_t */
+    double rel_tol;          /* tau */
+    double eta;              /* re-orthogonalisation threshold; 0 -> 1/sqrt(2) (reading Q3) */
+    double *h_res_history;   /* optional HOST buffer: recurrence residual |g_{j+1}|/||b|| per Arnoldi step */
+    int32_t res_history_cap; /* entries available in h_res_history (0 if unused) */
+    int32_t reserved;
+} cbgmres_params;
+
+typedef struct {
+    int32_t iters;        /* Arnoldi steps done */
+    int32_t restarts;     /* restart cycles started */
+    int32_t reorth_count; /* steps on which the second Gram-Schmidt pass ran */
+    int32_t breakdown;    /* 1 if the last cycle ended through Fig. 1 line 12 */
+    int32_t converged;    /* 1 iff the explicit residual met tau*||b|| */
+    int32_t spmv_kernel;  /* which SpMV variant ran (see cbgmres_set_option "spmv_kernel") */
+    double rel_res_recurrence; /* |g_{k+1}| / ||b|| at the end of the last cycle */
+    double rel_res_true;       /* last explicit ||b - A x|| / ||b|| */
+    double b_norm;
+    double solve_ms;      /* device time of the whole solve (CUDA events on the stream) */
+} cbgmres_result;
+
+/* ---- the four calls of the problem statement ------------------------------------------------ */
+
+/* Create a handle bound to `device` and to `cuda_stream` (a cudaStream_t, borrowed; NULL = the
+ * legacy default stream).  Allocates the handle's fixed scratch block. */
+int cbgmres_create(cbgmres_handle_t *out, int device, void *cuda_stream);
+
+/* Register A in CSR: row_ptr int32[n+1], col_idx int32[nnz], vals fp64[nnz], all
+ * DEVICE, BORROWED (not copied).  Reads row_ptr once (synchronises the stream) to choose the SpMV
+ * variant for the row-length distribution ("automatically selects a CSR kernel"). */
+int cbgmres_set_matrix(cbgmres_handle_t h, int64_t n, int64_t nnz, const int32_t *d_row_ptr,
+                       const int32_t *d_col_idx, const double *d_vals);
+
+/* Bytes of device workspace cbgmres_solve needs for these params and the registered matrix:
+ * (restart+1) basis vectors in the storage format + two fp64 work vectors + small arrays. */
+int cbgmres_workspace_bytes(cbgmres_handle_t h, const cbgmres_params *p, size_t *bytes);
+
+/* Restarted CB-GMRES (Fig. 1).  d_b fp64[n]; d_x fp64[n] holds x0 on entry and the solution
+ * approximation on exit; d_workspace 256-byte aligned.  Synchronises the stream, fills *out.
+ * Returns CBGMRES_OK (converged), CBGMRES_NOT_CONVERGED, or an error. */
+int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgmres_params *p, void *d_workspace,
+                  size_t workspace_bytes, cbgmres_result *out);
+
+/* Same solve with HOST buffers (the end-to-end path bench.py times): copies the CSR arrays, b and
+ * x0 host->device into the workspace, solves, copies x device->host.  Needs
+ * cbgmres_workspace_bytes_host bytes.  Host buffers should be pinned for full copy bandwidth.
+ * Replaces the handle's registered matrix (it then points into d_workspace). */
+int cbgmres_workspace_bytes_host(cbgmres_handle_t h, int64_t n, int64_t nnz, const cbgmres_params *p, size_t *bytes);
+int cbgmres_solve_host(cbgmres_handle_t h, int64_t n, int64_t nnz, const int32_t *h_row_ptr, const int32_t *h_col_idx,
+                       const double *h_vals, const double *h_b, double *h_x, const cbgmres_params *p,
+                       void *d_workspace, size_t workspace_bytes, cbgmres_result *out);
+
+int cbgmres_destroy(cbgmres_handle_t h);
+
+/* Static string describing the last error on this handle (valid until the next call). */
+const char *cbgmres_last_error(cbgmres_handle_t h);
+
+/* Tuning / test knobs, by name.  "spmv_kernel": 0 = choose from the row-length statistics,
+ * L in {2,4,8,16,32} = L lanes per row, 64 = nnz-balanced streaming kernel.  "poll": 1 (default)
+ * = the host stops launching a cycle's remaining steps once the device reports it left the cycle.
+ * Unknown names return CBGMRES_E_INVALID. */
+int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value);
+
+/* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
+int64_t cbgmres_launch_count(cbgmres_handle_t h);
+
+/* ---- per-kernel hooks (parity is judged per kernel: BASELINE.json north_star) ------------- */
+
+/* enc: d_payload[n] <- storage(d_v[n]); *d_scale <- sigma (1.0 for the
+ * floating-point formats).  Bit-exact function of the fp64 input. */
+int cbgmres_k_compress(cbgmres_handle_t h, int32_t format, int64_t n, const double *d_v, void *d_payload,
+                       double *d_scale);
+/* dec: d_v[n] <- fp64(d_payload[n]) * (*d_scale for the integer formats). */
+int cbgmres_k_decode(cbgmres_handle_t h, int32_t format, int64_t n, const void *d_payload, const double *d_scale,
+                     double *d_v);
+/* S2, Fig. 1 line 5: d_h[c] <- sum_i dec(V)[i,c] * d_w[i], c = 0..k-1. */
+int cbgmres_k_multidot(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld, int32_t k, const void *d_V,
+                       const double *d_scales, const double *d_w, double *d_h);
+/* S3, Fig. 1 lines 5-6: d_w[i] <- d_w[i] - sum_c dec(V)[i,c] * d_h[c];
+ * *d_nrm2 <- ||w||_2 and *d_amax <- ||w||_inf of the new w, computed in the same pass. */
+int cbgmres_k_update(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld, int32_t k, const void *d_V,
+                     const double *d_scales, const double *d_h, double *d_w, double *d_nrm2, double *d_amax);
+/* S4, Fig. 1 lines 13-14: d_v_fp64[i] <- d_w[i] / hnorm;
+ * d_payload_col[n] <- enc(v); *d_scale <- sigma.  amax = ||w||_inf (only read by the integer formats). */
+int cbgmres_k_store(cbgmres_handle_t h, int32_t format, int64_t n, const double *d_w, double hnorm, double amax,
+                    void *d_payload_col, double *d_scale, double *d_v_fp64);
+/* S1, Fig. 1 line 3: d_w <- A d_v with the registered matrix; if d_nrm2 != NULL,
+ * *d_nrm2 <- ||w||_2 (omega, line 4) from the same pass. */
+int cbgmres_k_spmv(cbgmres_handle_t h, const double *d_v, double *d_w, double *d_nrm2);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CBGMRES_H_ */

@@ -88,16 +88,22 @@ static uint16_t f64_to_f16_bits(double x)
     return (uint16_t)(sign | bits);
 }
 
+/* binary16 -> binary64 is exact.  Normal halves: same sign, exponent re-biased (e - 15 + 1023), the
+ * 10 fraction bits become the top 10 of the 52.  Subnormal halves: m * 2^-24. */
 static double f16_bits_to_f64(uint16_t h)
 {
-    int s = (h >> 15) & 1;
-    int e = (h >> 10) & 0x1F;
-    int m = h & 0x3FF;
+    const uint64_t s = (uint64_t)(h >> 15) & 1u;
+    const int e = (h >> 10) & 0x1F;
+    const uint64_t m = h & 0x3FFu;
     double v;
-    if (e == 0) v = ldexp((double)m, -24);
-    else if (e == 31) v = m ? NAN : INFINITY;
-    else v = ldexp((double)(1024 + m), e - 25);
-    return s ? -v : v;
+    if (e == 0) {
+        v = (double)m * 0x1p-24;
+        return s ? -v : v;
+    }
+    if (e == 31) return m ? NAN : (s ? -INFINITY : INFINITY);
+    const uint64_t bits = (s << 63) | ((uint64_t)(e - 15 + 1023) << 52) | (m << 42);
+    memcpy(&v, &bits, 8);
+    return v;
 }
 
 /* enc: fp64[n] -> (payload, sigma).  sigma is 1 for the floating-point formats.
@@ -114,12 +120,14 @@ int orc_enc(int fmt, int64_t n, const double *v, void *payload, double *sigma)
         return 0;
     case ORC_F32: {
         float *p = (float *)payload;
+#pragma omp parallel for schedule(static)
         for (i = 0; i < n; i++) p[i] = (float)v[i]; /* cvtsd2ss: RNE, gradual underflow */
         *sigma = 1.0;
         return 0;
     }
     case ORC_F16: {
         uint16_t *p = (uint16_t *)payload;
+#pragma omp parallel for schedule(static)
         for (i = 0; i < n; i++) p[i] = f64_to_f16_bits(v[i]);
         *sigma = 1.0;
         return 0;
@@ -138,6 +146,7 @@ int orc_enc(int fmt, int64_t n, const double *v, void *payload, double *sigma)
             return 0;
         }
         double s = maxint / a;
+#pragma omp parallel for schedule(static)
         for (i = 0; i < n; i++) {
             double q = nearbyint(v[i] * s); /* default rounding mode: to nearest, ties to even */
             if (q > maxint) q = maxint;
@@ -160,10 +169,22 @@ int orc_dec(int fmt, int64_t n, const void *payload, double sigma, double *out)
     int64_t i;
     switch (fmt) {
     case ORC_F64: memcpy(out, payload, (size_t)n * 8); return 0;
-    case ORC_F32: for (i = 0; i < n; i++) out[i] = (double)((const float *)payload)[i]; return 0;
-    case ORC_F16: for (i = 0; i < n; i++) out[i] = f16_bits_to_f64(((const uint16_t *)payload)[i]); return 0;
-    case ORC_I32: for (i = 0; i < n; i++) out[i] = (double)((const int32_t *)payload)[i] * sigma; return 0;
-    case ORC_I16: for (i = 0; i < n; i++) out[i] = (double)((const int16_t *)payload)[i] * sigma; return 0;
+    case ORC_F32:
+#pragma omp parallel for schedule(static)
+        for (i = 0; i < n; i++) out[i] = (double)((const float *)payload)[i];
+        return 0;
+    case ORC_F16:
+#pragma omp parallel for schedule(static)
+        for (i = 0; i < n; i++) out[i] = f16_bits_to_f64(((const uint16_t *)payload)[i]);
+        return 0;
+    case ORC_I32:
+#pragma omp parallel for schedule(static)
+        for (i = 0; i < n; i++) out[i] = (double)((const int32_t *)payload)[i] * sigma;
+        return 0;
+    case ORC_I16:
+#pragma omp parallel for schedule(static)
+        for (i = 0; i < n; i++) out[i] = (double)((const int16_t *)payload)[i] * sigma;
+        return 0;
     default: return -1;
     }
 }
@@ -184,12 +205,29 @@ void orc_spmv(int64_t n, const int32_t *rp, const int32_t *ci, const double *va,
     }
 }
 
+/* Dot product.  Each thread sums one contiguous block of the index range (static schedule) and
+ * the per-thread sums are added in thread order, so the result is reproducible run to run for a
+ * fixed thread count (an OpenMP reduction clause leaves the combination order unspecified). */
+#define ORC_MAX_THREADS 1024
 static double dot(int64_t n, const double *a, const double *b)
 {
+    double part[ORC_MAX_THREADS];
+    int nt = 1;
+#pragma omp parallel
+    {
+#ifdef _OPENMP
+        const int t = omp_get_thread_num(), T = omp_get_num_threads();
+#else
+        const int t = 0, T = 1;
+#endif
+        const int64_t lo = n * t / T, hi = n * (t + 1) / T;
+        double s = 0.0;
+        for (int64_t i = lo; i < hi; i++) s += a[i] * b[i];
+        part[t] = s;
+        if (t == 0) nt = T;
+    }
     double s = 0.0;
-    int64_t i;
-#pragma omp parallel for schedule(static) reduction(+ : s)
-    for (i = 0; i < n; i++) s += a[i] * b[i];
+    for (int t = 0; t < nt; t++) s += part[t];
     return s;
 }
 

@@ -1,0 +1,211 @@
+// device_utils.cuh -- storage-format traits (decode in registers), encoders, warp/block
+// reductions and the last-block-done ticket used by every reduction kernel.
+#pragma once
+#include "internal.cuh"
+
+namespace cbg {
+
+// ---- 128-bit streaming loads -------------------------------------------------------------------
+// Basis payloads are read once per kernel: bypass L1 allocation, keep the default L2 policy so
+// that the update pass can still find the multi-dot pass's lines in the 126 MB L2.
+__device__ __forceinline__ uint4 ldg_stream128(const void *p)
+{
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p));
+    return r;
+}
+
+// ---- storage formats ----------------------------------------------------------
+// VEC = entries per 128-bit load.  decode() widens one 128-bit payload word to VEC fp64 values
+// WITHOUT the per-vector scale: the fixed-point scale sigma_c is folded into the coefficient
+// (h_c = sigma_c * sum q w ; w -= sum q (sigma_c h_c)), so the "one multiplication per element"
+// of PAPER.md:181 disappears from the inner loops.
+template <int FMT> struct Fmt;
+
+template <> struct Fmt<CBGMRES_FP64> {
+    static constexpr int VEC = 2, BYTES = 8;
+    static constexpr bool SCALED = false;
+    __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
+    {
+        d[0] = __hiloint2double((int)r.y, (int)r.x);
+        d[1] = __hiloint2double((int)r.w, (int)r.z);
+    }
+    __device__ static __forceinline__ double decode_one(const void *col, int64_t i) { return ((const double *)col)[i]; }
+};
+
+template <> struct Fmt<CBGMRES_FP32> {
+    static constexpr int VEC = 4, BYTES = 4;
+    static constexpr bool SCALED = false;
+    __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
+    {
+        d[0] = (double)__uint_as_float(r.x);
+        d[1] = (double)__uint_as_float(r.y);
+        d[2] = (double)__uint_as_float(r.z);
+        d[3] = (double)__uint_as_float(r.w);
+    }
+    __device__ static __forceinline__ double decode_one(const void *col, int64_t i)
+    {
+        return (double)((const float *)col)[i];
+    }
+};
+
+__device__ __forceinline__ void half2_to_doubles(unsigned w, double &lo, double &hi)
+{
+    const __half2 h = *reinterpret_cast<const __half2 *>(&w);
+    const float2 f = __half22float2(h); // exact widening
+    lo = (double)f.x;
+    hi = (double)f.y;
+}
+
+template <> struct Fmt<CBGMRES_FP16> {
+    static constexpr int VEC = 8, BYTES = 2;
+    static constexpr bool SCALED = false;
+    __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
+    {
+        half2_to_doubles(r.x, d[0], d[1]);
+        half2_to_doubles(r.y, d[2], d[3]);
+        half2_to_doubles(r.z, d[4], d[5]);
+        half2_to_doubles(r.w, d[6], d[7]);
+    }
+    __device__ static __forceinline__ double decode_one(const void *col, int64_t i)
+    {
+        return (double)__half2float(((const __half *)col)[i]);
+    }
+};
+
+template <> struct Fmt<CBGMRES_INT32> {
+    static constexpr int VEC = 4, BYTES = 4;
+    static constexpr bool SCALED = true;
+    __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
+    {
+        d[0] = (double)(int)r.x;
+        d[1] = (double)(int)r.y;
+        d[2] = (double)(int)r.z;
+        d[3] = (double)(int)r.w;
+    }
+    __device__ static __forceinline__ double decode_one(const void *col, int64_t i)
+    {
+        return (double)((const int32_t *)col)[i];
+    }
+};
+
+template <> struct Fmt<CBGMRES_INT16> {
+    static constexpr int VEC = 8, BYTES = 2;
+    static constexpr bool SCALED = true;
+    __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
+    {
+        const unsigned w[4] = {r.x, r.y, r.z, r.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            d[2 * i] = (double)(int)(short)(w[i] & 0xFFFFu);
+            d[2 * i + 1] = (double)((int)w[i] >> 16);
+        }
+    }
+    __device__ static __forceinline__ double decode_one(const void *col, int64_t i)
+    {
+        return (double)((const int16_t *)col)[i];
+    }
+};
+
+// ---- encoders (bit-exact functions of the fp64 input; readings Q6-Q8) ----------------
+// s = max_int / a for the fixed-point formats (unused otherwise).
+template <int FMT> __device__ __forceinline__ unsigned enc_bits(double v, double s);
+template <> __device__ __forceinline__ unsigned enc_bits<CBGMRES_FP32>(double v, double)
+{
+    return __float_as_uint(__double2float_rn(v)); // cvt.rn.f32.f64, no .ftz: gradual underflow
+}
+template <> __device__ __forceinline__ unsigned enc_bits<CBGMRES_FP16>(double v, double)
+{
+    return (unsigned)__half_as_ushort(__double2half(v)); // cvt.rn.f16.f64: ONE rounding
+}
+template <> __device__ __forceinline__ unsigned enc_bits<CBGMRES_INT32>(double v, double s)
+{
+    int q = __double2int_rn(__dmul_rn(v, s)); // ties to even; saturates
+    q = max(q, -2147483647);                  // symmetric clamp (reading Q6)
+    return (unsigned)q;
+}
+template <> __device__ __forceinline__ unsigned enc_bits<CBGMRES_INT16>(double v, double s)
+{
+    int q = __double2int_rn(__dmul_rn(v, s));
+    q = min(max(q, -32767), 32767);
+    return (unsigned)q & 0xFFFFu;
+}
+
+template <int FMT> __device__ __forceinline__ double fmt_maxint()
+{
+    return FMT == CBGMRES_INT32 ? 2147483647.0 : 32767.0;
+}
+
+// ---- reductions ---------------------------------------------------------------------------------
+__device__ __forceinline__ double shfl_xor_f64(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += shfl_xor_f64(v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, shfl_xor_f64(v, o));
+    return v;
+}
+
+// Transposing butterfly: every lane holds N partial sums (one per column); afterwards lane L with
+// (L % (32/N)) == 0 holds the warp total of column butterfly_col<N>(L).  N + log2(32/N) - 1
+// shuffles instead of 5 N.  Summation order is fixed, so results are reproducible.
+template <int N, int OFF> __device__ __forceinline__ double butterfly_rec(double (&a)[N], int lane)
+{
+    if constexpr (N == 1) {
+        double v = a[0];
+#pragma unroll
+        for (int o = OFF; o > 0; o >>= 1) v += shfl_xor_f64(v, o);
+        return v;
+    } else {
+        constexpr int H = N / 2;
+        const bool up = (lane & OFF) != 0;
+        double b[H];
+#pragma unroll
+        for (int i = 0; i < H; ++i) {
+            const double send = up ? a[i] : a[i + H];
+            const double keep = up ? a[i + H] : a[i];
+            b[i] = keep + shfl_xor_f64(send, OFF);
+        }
+        return butterfly_rec<H, OFF / 2>(b, lane);
+    }
+}
+
+// Column held by lane L after butterfly_rec<N,16>: the top log2(N) bits of L, MSB first.
+template <int N> __device__ __forceinline__ int butterfly_col(int lane)
+{
+    int col = 0, off = 16;
+#pragma unroll
+    for (int h = N / 2; h >= 1; h >>= 1) {
+        if (lane & off) col += h;
+        off >>= 1;
+    }
+    return col;
+}
+template <int N> __device__ __forceinline__ bool butterfly_owner(int lane) { return (lane & (32 / N - 1)) == 0; }
+
+// Last-block-done ticket: returns true in every thread of the CTA that arrives last.  Partials
+// written before the call are visible to that CTA.  The counter is reset for the next launch.
+__device__ __forceinline__ bool last_block_done(unsigned *ticket)
+{
+    __shared__ int s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned t = atomicAdd(ticket, 1u);
+        s_last = (t == gridDim.x - 1);
+        if (s_last) *ticket = 0u;
+    }
+    __syncthreads();
+    if (s_last) __threadfence();
+    return s_last != 0;
+}
+
+} // namespace cbg

@@ -1,0 +1,106 @@
+// internal.cuh -- shared declarations of the CB-GMRES CUDA library (sm_100a only).
+// Nothing in this tree is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+
+#include "../../include/cbgmres.h"
+
+namespace cbg {
+
+constexpr int kMaxRestart = CBGMRES_MAX_RESTART;
+constexpr int kNumSMs = 148;           // B200: 2 dies x 74 SMs
+constexpr int kMaxGrid = kNumSMs * 8;  // upper bound on CTAs of any reduction kernel (partials rows)
+constexpr int kLdp = kMaxRestart + 8;  // leading dimension of the multi-dot partials matrix
+
+// Step kinds: the guard every step kernel evaluates from the device-resident control block.
+enum Mode : int {
+    MODE_HOOK = 0,     // per-kernel test hook: no guard, no solver control
+    MODE_ORTH1 = 1,    // first Gram-Schmidt pass of Arnoldi step `step`   (Fig. 1 l.5-6)
+    MODE_ORTH2 = 2,    // conditional second pass                           (Fig. 1 l.7-11)
+    MODE_XUPDATE = 3,  // x += V_k y at the end of a cycle                  (Fig. 1 l.17)
+    MODE_RESIDUAL = 4, // r = b - A x at the start of a cycle               (Fig. 1 l.1)
+    MODE_STEP = 5,     // w = A v of Arnoldi step `step`                    (Fig. 1 l.3-4)
+    MODE_BNORM = 6,    // ||b|| once per solve
+};
+
+// Device-resident control block: every scalar the Arnoldi loop decides on lives here, so the
+// host launches a whole restart cycle without reading anything back (one sync per cycle).
+struct Ctl {
+    // reduction results
+    double sumsq_w;   // sum w_i^2 after the SpMV (omega^2) or of the explicit residual
+    double amax_w;    // max |w_i| of the explicit residual (feeds the store of V[:,0])
+    double omega;     // ||A v||_2 of the current step (Fig. 1 l.4)
+    double hn;        // h_{j+1,j} (or beta at cycle start): the divisor of the next store
+    double amax;      // ||w||_inf matching hn
+    double hook_nrm2; // outputs of the k_update hook
+    double hook_amax;
+    // solve-wide scalars
+    double bnorm, tol_abs, beta, eta, rel_rec, rel_true, rel_tol;
+    // control
+    int stop_after;   // Arnoldi steps with index > stop_after are skipped in this cycle
+    int reorth_flag;  // set by the first pass's finalisation, read by the second pass
+    int k;            // Arnoldi steps completed in the current cycle
+    int iters, max_iters, reorth_count, breakdown, converged, nonfinite, restarts, done;
+    int reorth_mode, m, hist_cap;
+    unsigned tickets[8]; // last-block-done counters, one per kernel family
+};
+
+// Small dense state of one restart cycle (device memory, < 3 MB at m = 512).
+struct CycleState {
+    double *h;      // [m+2]  current Hessenberg column (h_{1:j,j}, then rotated in place)
+    double *hs;     // [m+2]  sigma_c * h_c: the coefficients the update kernel multiplies payloads with
+    double *R;      // [(m+1) * m] rotated Hessenberg, column-major, ld = m+1
+    double *cs, *sn; // [m] Givens rotations
+    double *g;      // [m+1] rotated right-hand side
+    double *y;      // [m]
+    double *scales; // [m+1] sigma_c per stored basis vector
+    double *hist;   // [hist_cap] recurrence residual per Arnoldi step
+};
+
+struct Scratch {
+    Ctl *ctl;          // device
+    double *partials;  // [kMaxGrid * kLdp] multi-dot partial sums, row = CTA
+    double *npart;     // [2 * kMaxGrid] sum-of-squares and max partials
+};
+
+struct BasisView {
+    const void *V;     // payload, vector-major
+    int64_t ld;        // entries per stored vector
+    const double *scales;
+    int format;
+};
+
+struct CsrView {
+    int64_t n, nnz;
+    const int32_t *row_ptr, *col_idx;
+    const double *vals;
+    const int32_t *blk_row; // [nblk+1] row partition of the streaming kernel (may be null)
+    int nblk;
+    int kernel;             // 2,4,8,16,32 lanes per row, or 64 = streaming
+};
+
+// ---- launchers (each enqueues on `s` and returns the number of kernels launched) -------------
+int launch_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t n, int k, const double *w,
+                    double *h_out, double *hs_out, int mode, int step);
+int launch_update(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t n, int k, const int *d_k,
+                  const double *hs, double *w, int mode, int step);
+int launch_store(cudaStream_t s, const Scratch &sc, int format, int64_t n, const double *w, const double *d_hn,
+                 const double *d_amax, double hn_host, double amax_host, void *payload_col, double *scale_out,
+                 double *v_out, int mode, int step, const CycleState *cyc, int *h_flag);
+int launch_decode(cudaStream_t s, int format, int64_t n, const void *payload, const double *d_scale, double *v);
+int launch_spmv(cudaStream_t s, const Scratch &sc, const CsrView &A, const double *x, const double *b, double *w,
+                int mode, int step, const CycleState *cyc, int *h_flag);
+int launch_nrm2(cudaStream_t s, const Scratch &sc, int64_t n, const double *x, int mode);
+int launch_backsolve(cudaStream_t s, const Scratch &sc, const CycleState &cyc, int format);
+int launch_scale_coeffs(cudaStream_t s, int k, const double *h, const double *scales, double *hs);
+int launch_copy_scalars(cudaStream_t s, const double *src0, double *dst0, const double *src1, double *dst1);
+
+int launch_row_stats(cudaStream_t s, int64_t n, const int32_t *d_row_ptr, int *d_out);
+
+// row-partition metadata for the streaming SpMV (set_matrix)
+cudaError_t build_row_blocks(cudaStream_t s, int64_t n, int64_t nnz, const int32_t *d_row_ptr, int nnz_per_block,
+                             int32_t **d_blk_row_out, int *nblk_out);
+
+} // namespace cbg

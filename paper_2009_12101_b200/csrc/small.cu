@@ -1,0 +1,64 @@
+// small.cu -- the tiny dense pieces that stay on the device (north_star: "small Hessenberg Givens
+// rotations and the triangular solve, kept on the device"): the back substitution R y = g of
+// Fig. 1 line 17 and two marshalling kernels used by the per-kernel hooks.
+#include "device_utils.cuh"
+
+namespace cbg {
+
+// One warp.  Column-oriented back substitution on the k x k upper-triangular R (column-major,
+// ld = m+1): y_i = g_i / R_ii, then g_{0..i-1} -= R_{0..i-1,i} y_i with the lanes striding the rows.
+// Leaves hs_c = -sigma_c * y_c, the coefficients with which the update kernel forms x += V_k y.
+template <bool SCALED> __global__ void __launch_bounds__(32) backsolve_kernel(Ctl *ctl, CycleState cy)
+{
+    const int k = ctl->k;
+    if (k <= 0) return;
+    __shared__ double t[kMaxRestart + 1];
+    const int lane = threadIdx.x, m = ctl->m;
+    for (int i = lane; i < k; i += 32) t[i] = cy.g[i];
+    __syncwarp();
+    for (int i = k - 1; i >= 0; --i) {
+        const double *Rc = cy.R + (size_t)i * (m + 1);
+        const double yi = t[i] / Rc[i];
+        __syncwarp();
+        if (lane == 0) t[i] = yi;
+        for (int l = lane; l < i; l += 32) t[l] = fma(-Rc[l], yi, t[l]);
+        __syncwarp();
+    }
+    for (int i = lane; i < k; i += 32) {
+        cy.y[i] = t[i];
+        cy.hs[i] = -(SCALED ? cy.scales[i] : 1.0) * t[i];
+    }
+}
+
+int launch_backsolve(cudaStream_t s, const Scratch &sc, const CycleState &cyc, int format)
+{
+    if (format == CBGMRES_INT32 || format == CBGMRES_INT16) backsolve_kernel<true><<<1, 32, 0, s>>>(sc.ctl, cyc);
+    else backsolve_kernel<false><<<1, 32, 0, s>>>(sc.ctl, cyc);
+    return 1;
+}
+
+__global__ void scale_coeffs_kernel(int k, const double *h, const double *scales, double *hs)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c < k) hs[c] = scales ? h[c] * scales[c] : h[c];
+}
+
+int launch_scale_coeffs(cudaStream_t s, int k, const double *h, const double *scales, double *hs)
+{
+    scale_coeffs_kernel<<<(k + 127) / 128, 128, 0, s>>>(k, h, scales, hs);
+    return 1;
+}
+
+__global__ void copy_scalars_kernel(const double *s0, double *d0, const double *s1, double *d1)
+{
+    if (d0 && s0) *d0 = *s0;
+    if (d1 && s1) *d1 = *s1;
+}
+
+int launch_copy_scalars(cudaStream_t s, const double *src0, double *dst0, const double *src1, double *dst1)
+{
+    copy_scalars_kernel<<<1, 1, 0, s>>>(src0, dst0, src1, dst1);
+    return 1;
+}
+
+} // namespace cbg

@@ -1,0 +1,245 @@
+"""GPU parity, per kernel, through the C ABI (BASELINE.json north_star): compression of a given fp64
+vector is bit-exact; dot / update / SpMV agree with the oracle's extended-precision references to
+1e-12 in the norm-wise metrics of DESIGN.md."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_config, ortho_basis
+
+pytestmark = pytest.mark.gpu
+
+FORMATS = oracle.FORMATS
+TOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def solver():
+    from paper_2009_12101_b200 import Solver
+
+    s = Solver(0)
+    yield s
+    s.destroy()
+
+
+def _dev(a, dtype=None):
+    import torch
+
+    t = torch.as_tensor(np.ascontiguousarray(a), device="cuda")
+    return t if dtype is None else t.to(dtype)
+
+
+def _basis(fmt, n, k, seed, ld_extra=0):
+    """k unit vectors (orthonormalised Gaussian), oracle-encoded, laid out [k, ld] on host and device."""
+    import torch
+
+    V, w = ortho_basis(n, k, seed=seed)
+    P, sig = oracle.enc_basis(fmt, V)
+    ld = (n + 63) // 64 * 64 + ld_extra
+    Ppad = np.zeros((k, ld), dtype=P.dtype)
+    Ppad[:, :n] = P
+    # poison the padding: the kernels must never let entries at or beyond n reach a result
+    if P.dtype.kind == "f":
+        Ppad[:, n:] = np.nan
+    else:
+        Ppad[:, n:] = np.iinfo(P.dtype).max
+    from paper_2009_12101_b200 import payload_dtype
+
+    dP = torch.as_tensor(Ppad, device="cuda").view(payload_dtype(fmt))
+    return Ppad, sig, w, dP, _dev(sig)
+
+
+# ------------------------------------------------------------------------------------------ codecs
+@pytest.mark.parametrize("fmt", FORMATS)
+@pytest.mark.parametrize("n", [1, 7, 64, 1000, 100003])
+def test_compress_bit_exact(solver, fmt, n):
+    rng = np.random.default_rng(100 + n)
+    w = rng.standard_normal(n)
+    v = w / np.linalg.norm(w)
+    if n > 20:  # ties, zeros, tiny values, the extremes
+        v[3] = 0.0
+        v[5] = -0.0
+        v[7] = 1e-30
+        v[11] = 2.0 ** -25
+        v[13] = -(2.0 ** -24 + 2.0 ** -25)
+    exp_p, exp_s = oracle.enc(fmt, v)
+    p, s = solver.k_compress(fmt, _dev(v))
+    got = p.cpu().numpy()
+    assert got.dtype == exp_p.dtype
+    assert np.array_equal(got.view(np.uint8), exp_p.view(np.uint8))
+    assert s.item() == exp_s
+    d = solver.k_decode(fmt, p, s).cpu().numpy()
+    assert np.array_equal(d, oracle.dec(fmt, exp_p, exp_s))
+
+
+@pytest.mark.parametrize("fmt", ["fp16", "fp32"])
+def test_compress_midpoints_and_subnormals(solver, fmt):
+    if fmt == "fp16":
+        bits = np.arange(0, 0x7BFF, dtype=np.uint16)
+        a = bits.view(np.float16).astype(np.float64)
+        up = (bits + 1).astype(np.uint16).view(np.float16).astype(np.float64)
+    else:
+        a32 = np.abs(np.random.default_rng(5).uniform(-1, 1, 50000).astype(np.float32))
+        a32 = np.concatenate([a32, np.float32([0.0, 1e-45, 1.1754942e-38, 1.17549435e-38])])
+        a = a32.astype(np.float64)
+        up = np.nextafter(a32, np.float32(np.inf)).astype(np.float64)
+    mid = (a + up) / 2
+    v = np.concatenate([mid, -mid, np.nextafter(mid, 0.0), np.nextafter(mid, np.inf)])
+    exp_p, _ = oracle.enc(fmt, v)
+    p, _ = solver.k_compress(fmt, _dev(v))
+    assert np.array_equal(p.cpu().numpy().view(np.uint8), exp_p.view(np.uint8))
+
+
+@pytest.mark.parametrize("fmt", ["int16", "int32"])
+def test_compress_fixed_point_ties_and_zero_vector(solver, fmt):
+    M = 32767 if fmt == "int16" else 2147483647
+    a = M * 2.0 ** -40
+    ties = np.array([0.5, 1.5, 2.5, -0.5, -1.5, -2.5, M - 0.5, -(M - 0.5), 3.25, -3.75]) * 2.0 ** -40
+    v = np.concatenate([[a, -a], ties])
+    exp_p, exp_s = oracle.enc(fmt, v)
+    p, s = solver.k_compress(fmt, _dev(v))
+    assert np.array_equal(p.cpu().numpy(), exp_p) and s.item() == exp_s == 2.0 ** -40
+    z, sz = solver.k_compress(fmt, _dev(np.zeros(100)))
+    assert not z.cpu().numpy().any() and sz.item() == 0.0
+
+
+# ------------------------------------------------------------------------------------------ store
+@pytest.mark.parametrize("fmt", FORMATS)
+@pytest.mark.parametrize("n", [5, 4099, 70001])
+def test_store_normalises_and_compresses(solver, fmt, n):
+    rng = np.random.default_rng(200 + n)
+    w = rng.standard_normal(n) * 37.5
+    hn = float(np.linalg.norm(w))
+    amax = float(np.abs(w).max())
+    v = w / hn  # IEEE division per element (reading Q8)
+    exp_p, exp_s = oracle.enc(fmt, v)
+    p, s, vout = solver.k_store(fmt, _dev(w), hn, amax)
+    assert np.array_equal(vout.cpu().numpy(), v)
+    assert np.array_equal(p.cpu().numpy().view(np.uint8), exp_p.view(np.uint8))
+    assert s.item() == exp_s
+
+
+# ------------------------------------------------------------------------------------------ multi-dot / update
+@pytest.mark.parametrize("fmt", FORMATS)
+@pytest.mark.parametrize("n,k", [(1, 1), (63, 3), (4096, 8), (50021, 1), (50021, 9), (50021, 33), (200003, 100)])
+def test_multidot_matches_oracle(solver, fmt, n, k):
+    k = min(k, n)
+    P, sig, w, dP, dsig = _basis(fmt, n, k, seed=300 + n + k, ld_extra=64)
+    h_ref = oracle.ref_multidot(fmt, P, sig, w, k=k)
+    h = solver.k_multidot(fmt, dP, dsig, _dev(w), n=n, k=k).cpu().numpy()
+    Vhat_norm = np.array([np.linalg.norm(oracle.dec(fmt, P[c, :n], sig[c])) for c in range(k)])
+    assert np.all(np.isfinite(h))
+    assert np.all(np.abs(h - h_ref) <= TOL * Vhat_norm * np.linalg.norm(w))
+
+
+@pytest.mark.parametrize("fmt", FORMATS)
+@pytest.mark.parametrize("n,k", [(1, 1), (63, 3), (4096, 8), (50021, 1), (50021, 9), (50021, 33), (200003, 100)])
+def test_update_matches_oracle(solver, fmt, n, k):
+    import torch
+
+    k = min(k, n)
+    P, sig, w, dP, dsig = _basis(fmt, n, k, seed=400 + n + k)
+    h = np.random.default_rng(401).standard_normal(k)
+    w_ref, ss_ref, am_ref = oracle.ref_update(fmt, P[:k], sig[:k], h, w)
+    dw = _dev(w).clone()
+    out = solver.k_update(fmt, dP[:k], dsig[:k], _dev(h), dw, n=n)
+    torch.cuda.synchronize()
+    w_gpu = dw.cpu().numpy()
+    nrm2, amax = out.cpu().numpy()
+    scale = np.linalg.norm(w) + np.linalg.norm(h)  # ||w|| + ||V^|| ||h||, ||V^|| ~ 1
+    assert np.linalg.norm(w_gpu - w_ref) <= TOL * scale
+    assert abs(nrm2 - np.sqrt(ss_ref)) <= TOL * scale
+    assert amax == np.abs(w_gpu).max()
+
+
+@pytest.mark.parametrize("fmt", FORMATS)
+def test_cgs_closed_form(solver, fmt):
+    """w in span(V^): the dots return the coefficients and the update annihilates w."""
+    n, k = 30011, 16
+    P, sig, _, dP, dsig = _basis(fmt, n, k, seed=500)
+    Vhat = np.stack([oracle.dec(fmt, P[c, :n], sig[c]) for c in range(k)])
+    c = np.random.default_rng(501).standard_normal(k)
+    w = c @ Vhat
+    dw = _dev(w).clone()
+    h = solver.k_multidot(fmt, dP, dsig, dw, n=n, k=k)
+    G = Vhat @ Vhat.T
+    assert np.allclose(h.cpu().numpy(), G @ c, rtol=0, atol=1e-12 * np.linalg.norm(w))
+    if fmt == "fp64":
+        out = solver.k_update(fmt, dP, dsig, h, dw, n=n)
+        assert out.cpu().numpy()[0] <= 1e-12 * np.linalg.norm(w)
+
+
+# ------------------------------------------------------------------------------------------ SpMV
+@pytest.mark.parametrize("name,kw", [("C1", {}), ("C2", {"grid": 30}), ("C4", {"n": 60000}), ("C5", {"grid": 20})])
+@pytest.mark.parametrize("kernel", [0, 2, 4, 8, 16, 32, 64])
+def test_spmv_matches_oracle(name, kw, kernel):
+    from paper_2009_12101_b200 import Solver
+
+    p = make_config(name, **kw)
+    s = Solver(0)
+    try:
+        s.set_option("spmv_kernel", kernel)
+        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+        x = np.random.default_rng(600).standard_normal(p.A.n)
+        y_ref, rowabs = oracle.ref_spmv(p.A, x)
+        w, nrm = s.k_spmv(_dev(x))
+        y = w.cpu().numpy()
+        assert np.all(np.abs(y - y_ref) <= TOL * np.maximum(rowabs, 1e-300))
+        assert abs(nrm.item() - np.linalg.norm(y_ref)) <= TOL * np.linalg.norm(y_ref)
+    finally:
+        s.destroy()
+
+
+def test_spmv_empty_rows_and_long_rows():
+    """Degenerate CSR shapes: empty rows, one dense row longer than the streaming buffer."""
+    import scipy.sparse as sp
+
+    from paper_2009_12101_b200 import Solver
+    from workloads import CSR
+
+    rng = np.random.default_rng(601)
+    n = 9000
+    M = sp.random(n, n, density=0.0005, random_state=7, format="lil")
+    M[17, :] = rng.standard_normal(n)      # a full row (9000 > 6000-entry product buffer)
+    M[4000, :3000] = 1.0                   # a long row inside an otherwise sparse block
+    M[100:140, :] = 0.0                    # empty rows
+    M = sp.csr_matrix(M)
+    M.sort_indices()
+    A = CSR(n, M.indptr.astype(np.int32), M.indices.astype(np.int32), M.data.astype(np.float64))
+    x = rng.standard_normal(n)
+    y_ref, rowabs = oracle.ref_spmv(A, x)
+    for kernel in (0, 8, 32, 64):
+        s = Solver(0)
+        try:
+            s.set_option("spmv_kernel", kernel)
+            s.set_matrix(A.row_ptr, A.col_idx, A.vals)
+            y = s.k_spmv(_dev(x))[0].cpu().numpy()
+            assert np.all(np.abs(y - y_ref) <= TOL * np.maximum(rowabs, 1e-300) + 0.0)
+            assert np.all(y[100:140] == 0.0)
+        finally:
+            s.destroy()
+
+
+# ------------------------------------------------------------------------------------------ errors
+def test_invalid_arguments_return_status_codes(solver):
+    import torch
+
+    from paper_2009_12101_b200 import CbgmresError, Solver
+
+    s = Solver(0)
+    try:
+        with pytest.raises(CbgmresError) as e:
+            s.k_spmv(torch.zeros(4, dtype=torch.float64, device="cuda"), torch.zeros(4, dtype=torch.float64, device="cuda"))
+        assert e.value.code == 2  # E_NOMATRIX
+        V = torch.zeros((2, 72), dtype=torch.float16, device="cuda")  # ld*2 bytes not a multiple of 16
+        with pytest.raises(CbgmresError) as e:
+            s.k_multidot("fp16", V[:, :70].contiguous(), None, torch.zeros(60, dtype=torch.float64, device="cuda"))
+        assert e.value.code == 1
+        with pytest.raises(CbgmresError) as e:
+            s.k_multidot("int16", torch.zeros((2, 64), dtype=torch.int16, device="cuda"), None,
+                         torch.zeros(60, dtype=torch.float64, device="cuda"))
+        assert e.value.code == 1  # fixed point without scales
+        with pytest.raises(CbgmresError):
+            s.set_option("no_such_option", 1)
+    finally:
+        s.destroy()

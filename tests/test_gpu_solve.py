@@ -1,0 +1,186 @@
+"""GPU parity of the whole solver through cbgmres_solve (BASELINE.json north_star): iteration counts
+to convergence agree with the oracle within +-2 % (at least +-2 steps), final true relative residuals
+are both below the tolerance and within 10x of each other.  The true residual of the GPU's x is
+recomputed by the oracle's SpMV, never taken from the GPU's own report."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_config, random_dense_system
+
+pytestmark = pytest.mark.gpu
+
+
+def _solve_gpu(p, fmt, restart=None, rel_tol=None, max_iters=None, reorth="cond", history=False, x0=None):
+    from paper_2009_12101_b200 import Solver
+
+    s = Solver(0)
+    try:
+        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+        x, r = s.solve(p.b, p.x0 if x0 is None else x0, restart or p.restart, rel_tol or p.rel_tol,
+                       max_iters or p.max_iters, fmt, reorth=reorth, history=history)
+        return x.cpu().numpy(), r
+    finally:
+        s.destroy()
+
+
+def _true_rel_res(p, x):
+    return oracle.nrm2(p.b - oracle.spmv(p.A, x)) / oracle.nrm2(p.b)
+
+
+def _check_parity(p, fmt, restart=None, rel_tol=None, max_iters=None, reorth="cond"):
+    restart, rel_tol, max_iters = restart or p.restart, rel_tol or p.rel_tol, max_iters or p.max_iters
+    ref = oracle.gmres(p.A, p.b, p.x0, restart, rel_tol, max_iters, fmt, reorth=reorth)
+    x, r = _solve_gpu(p, fmt, restart, rel_tol, max_iters, reorth)
+    true_gpu = _true_rel_res(p, x)
+    true_ref = _true_rel_res(p, ref.x)
+    assert r.converged == ref.converged
+    assert abs(r.iters - ref.iters) <= max(2, 0.02 * ref.iters), (fmt, r.iters, ref.iters)
+    if ref.converged:
+        assert true_gpu <= rel_tol * (1 + 1e-9) and true_ref <= rel_tol * (1 + 1e-9)
+    assert true_gpu <= 10 * true_ref and true_ref <= 10 * true_gpu
+    assert r.rel_res_true == pytest.approx(true_gpu, rel=1e-6)
+    assert abs(r.restarts - ref.restarts) <= 1
+    assert r.b_norm == pytest.approx(ref.b_norm, rel=1e-13)
+    return r, ref
+
+
+@pytest.mark.parametrize("fmt", ["fp64", "fp32"])
+def test_c1_full_size(fmt):
+    p = make_config("C1")
+    r, ref = _check_parity(p, fmt)
+    assert r.converged
+
+
+@pytest.mark.parametrize("fmt", oracle.FORMATS)
+def test_c2_reduced(fmt):
+    _check_parity(make_config("C2", grid=32), fmt)
+
+
+@pytest.mark.parametrize("fmt", oracle.FORMATS)
+def test_c4_reduced(fmt):
+    # without a preconditioner C4 does not converge within its iteration bound (reading Q12); both
+    # sides must then stop at the bound with comparable true residuals
+    r, ref = _check_parity(make_config("C4", n=40000), fmt, max_iters=300)
+    assert r.iters == ref.iters == 300
+
+
+@pytest.mark.parametrize("fmt", oracle.FORMATS)
+def test_c5_reduced(fmt):
+    _check_parity(make_config("C5", grid=24), fmt)
+
+
+@pytest.mark.parametrize("reorth", ["never", "always"])
+def test_reorth_modes(reorth):
+    p = make_config("C2", grid=20)
+    r, ref = _check_parity(p, "fp32", restart=30, reorth=reorth)
+    assert (r.reorth_count == 0) if reorth == "never" else (r.reorth_count == r.iters)
+
+
+def test_recurrence_history_matches_oracle_first_cycle():
+    p = make_config("C2", grid=16)
+    ref = oracle.gmres(p.A, p.b, p.x0, 40, 1e-8, 400, "fp64")
+    x, r = _solve_gpu(p, "fp64", 40, 1e-8, 400, history=True)
+    k = min(30, r.iters, ref.iters)
+    assert np.allclose(r.rec_history[:k], ref.rec_history[:k], rtol=1e-6)
+
+
+def test_tiny_dense_matches_direct_solve():
+    for n, seed in ((1, 40), (3, 41), (33, 42), (64, 43)):
+        A, Ad, b = random_dense_system(n, seed)
+        from paper_2009_12101_b200 import Solver
+
+        s = Solver(0)
+        try:
+            s.set_matrix(A.row_ptr, A.col_idx, A.vals)
+            x, r = s.solve(b, np.zeros(n), n, 1e-13, 4 * n + 4, "fp64")
+            assert r.converged and r.iters <= n
+            xs = np.linalg.solve(Ad, b)
+            assert np.linalg.norm(x.cpu().numpy() - xs) <= 1e-10 * np.linalg.norm(xs)
+        finally:
+            s.destroy()
+
+
+def test_edge_cases_zero_rhs_exact_x0_max_iters_restart1():
+    p = make_config("C1", grid=16)
+    from paper_2009_12101_b200 import Solver
+
+    s = Solver(0)
+    try:
+        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+        x, r = s.solve(np.zeros(p.A.n), np.ones(p.A.n), 10, 1e-10, 50, "fp32")
+        assert r.converged and r.iters == 0 and not x.cpu().numpy().any()
+        xs = p.meta["xstar"]
+        x, r = s.solve(p.b, xs, 10, 1e-10, 50, "fp64")
+        assert r.converged and r.iters == 0 and r.restarts == 0 and np.array_equal(x.cpu().numpy(), xs)
+        x, r = s.solve(p.b, p.x0, 10, 1e-14, 25, "fp64")
+        assert (not r.converged) and r.status == 16 and r.iters == 25 and r.restarts == 3
+        ref = oracle.gmres(p.A, p.b, p.x0, 10, 1e-14, 25, "fp64")
+        assert _true_rel_res(p, x.cpu().numpy()) == pytest.approx(ref.rel_res_true, rel=1e-6)
+        # restart length 1 (GMRES(1)) still runs the whole path
+        x, r = s.solve(p.b, p.x0, 1, 1e-3, 500, "int16")
+        ref = oracle.gmres(p.A, p.b, p.x0, 1, 1e-3, 500, "int16")
+        assert r.converged == ref.converged and abs(r.iters - ref.iters) <= max(2, 0.02 * ref.iters)
+    finally:
+        s.destroy()
+
+
+def test_breakdown_on_invariant_subspace():
+    import scipy.sparse as sp
+
+    from paper_2009_12101_b200 import Solver
+    from workloads import CSR
+
+    n = 10
+    b = np.random.default_rng(44).standard_normal(n)
+    D = sp.csr_matrix(np.diag(np.full(n, 3.0)))
+    A = CSR(n, D.indptr.astype(np.int32), D.indices.astype(np.int32), D.data.astype(np.float64))
+    s = Solver(0)
+    try:
+        s.set_matrix(A.row_ptr, A.col_idx, A.vals)
+        x, r = s.solve(b, np.zeros(n), 5, 1e-12, 20, "fp64")
+        assert r.converged and r.iters == 1 and r.breakdown == 1
+        assert np.allclose(x.cpu().numpy(), b / 3.0, rtol=1e-15)
+    finally:
+        s.destroy()
+
+
+def test_solve_host_matches_device_solve():
+    import torch
+
+    from paper_2009_12101_b200 import Solver
+
+    p = make_config("C2", grid=24)
+    s = Solver(0)
+    try:
+        pin = lambda a: torch.as_tensor(a).pin_memory()
+        hx = pin(p.x0.copy())
+        r = s.solve_host(pin(p.A.row_ptr), pin(p.A.col_idx), pin(p.A.vals), pin(p.b), hx, p.restart, p.rel_tol,
+                         p.max_iters, "fp32")
+        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+        x, r2 = s.solve(p.b, p.x0, p.restart, p.rel_tol, p.max_iters, "fp32")
+        assert r.converged and r.iters == r2.iters
+        assert np.array_equal(hx.numpy(), x.cpu().numpy())  # deterministic reductions: bitwise repeatable
+        assert _true_rel_res(p, hx.numpy()) <= p.rel_tol
+    finally:
+        s.destroy()
+
+
+def test_invalid_solve_arguments():
+    from paper_2009_12101_b200 import CbgmresError, Solver
+
+    p = make_config("C1", grid=8)
+    s = Solver(0)
+    try:
+        with pytest.raises(CbgmresError) as e:
+            s.solve(p.b, p.x0, 10, 1e-8, 10, "fp64")
+        assert e.value.code == 2
+        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+        for kw in (dict(restart=0), dict(restart=513), dict(rel_tol=-1.0), dict(max_iters=-1)):
+            args = dict(restart=10, rel_tol=1e-8, max_iters=10)
+            args.update(kw)
+            with pytest.raises(CbgmresError) as e:
+                s.solve(p.b, p.x0, args["restart"], args["rel_tol"], args["max_iters"], "fp64")
+            assert e.value.code == 1
+    finally:
+        s.destroy()
