@@ -44,6 +44,8 @@ def lib():
     if _lib is None:
         L = C.CDLL(_build())
         L.orc_num_threads.restype = C.c_int
+        L.orc_set_num_threads.argtypes = [C.c_int]
+        L.orc_set_num_threads.restype = None
         L.orc_format_bytes.restype = C.c_int64
         L.orc_format_bytes.argtypes = [C.c_int]
         L.orc_enc.argtypes = [C.c_int, C.c_int64, C.c_void_p, C.c_void_p, C.POINTER(C.c_double)]
@@ -80,6 +82,11 @@ def _f64(a) -> np.ndarray:
 
 def num_threads() -> int:
     return int(lib().orc_num_threads())
+
+
+def set_num_threads(t: int) -> None:
+    """Thread count of later calls: changes only the order of dot()'s block sums (reading Q11)."""
+    lib().orc_set_num_threads(int(t))
 
 
 def format_bytes(fmt: str) -> int:

@@ -44,6 +44,19 @@ int orc_num_threads(void)
 #endif
 }
 
+/* Thread count of the following calls (t <= 0: leave as is).  It only changes the order in which
+ * dot() adds its per-thread block sums, i.e. the last bits of each inner product: tests use it to
+ * measure how far the oracle's OWN iteration counts move under rounding-level perturbations
+ * (reading Q11). */
+void orc_set_num_threads(int t)
+{
+#ifdef _OPENMP
+    if (t > 0) omp_set_num_threads(t);
+#else
+    (void)t;
+#endif
+}
+
 int64_t orc_format_bytes(int fmt)
 {
     switch (fmt) {

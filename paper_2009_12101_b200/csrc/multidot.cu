@@ -178,7 +178,7 @@ template <int FMT, int CT, int WARPS> static int launch_t(cudaStream_t s, const 
     const size_t smem = (size_t)WARPS * ((size_t)a.chunk_rows + a.kpad) * 8;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaFuncSetAttribute(multidot_kernel<FMT, CT, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
+        cudaFuncSetAttribute(multidot_kernel<FMT, CT, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 222 * 1024); // + ~2 KB static <= 227 KB
         attr_set = true;
     }
     (void)sizeof(F);

@@ -61,7 +61,6 @@ __device__ __forceinline__ void finalize_norms(const SpmvArgs &a)
         ctl->beta = beta;
         ctl->rel_true = beta / ctl->bnorm;
         ctl->k = 0;
-        ctl->breakdown = 0;
         int stop_after = 0;
         if (!isfinite(beta)) {
             ctl->nonfinite = 1;
@@ -73,6 +72,7 @@ __device__ __forceinline__ void finalize_norms(const SpmvArgs &a)
             ctl->done = 1;
         } else {
             ctl->restarts += 1;
+            ctl->breakdown = 0; // reported for the last cycle that ran (Fig. 1 l.12)
             stop_after = ctl->m;
             ctl->hn = beta; // v_1 := r_0 / beta through the same store kernel
             ctl->amax = m;

@@ -28,6 +28,29 @@ def _true_rel_res(p, x):
     return oracle.nrm2(p.b - oracle.spmv(p.A, x)) / oracle.nrm2(p.b)
 
 
+def _assert_iters_parity(gpu_iters, ref, p, fmt, restart, rel_tol, max_iters, reorth):
+    """+-2 % (at least +-2 steps) of the oracle's iteration count.  With a quantised basis the store
+    is a discontinuous map: a last-bit difference in one inner product flips rounding decisions and
+    the two residual histories decorrelate at the level of the storage format's unit roundoff after
+    some tens of steps (measured: DESIGN.md reading Q11).  Where the FIRST comparison fails, the
+    band is therefore widened to the spread of the oracle's OWN counts when only the order of its
+    block sums changes (thread counts 1, 2, 3, 5) -- nothing else about the oracle changes."""
+    tol = lambda c: max(2, 0.02 * c)
+    if abs(gpu_iters - ref.iters) <= tol(ref.iters):
+        return
+    assert fmt != "fp64", ("fp64 storage has no quantisation: no band", gpu_iters, ref.iters)
+    counts = [ref.iters]
+    base = oracle.num_threads()
+    try:
+        for t in (1, 2, 3, 5):
+            oracle.set_num_threads(t)
+            counts.append(oracle.gmres(p.A, p.b, p.x0, restart, rel_tol, max_iters, fmt, reorth=reorth).iters)
+    finally:
+        oracle.set_num_threads(base)
+    lo, hi = min(counts), max(counts)
+    assert lo - tol(lo) <= gpu_iters <= hi + tol(hi), (fmt, gpu_iters, counts)
+
+
 def _check_parity(p, fmt, restart=None, rel_tol=None, max_iters=None, reorth="cond"):
     restart, rel_tol, max_iters = restart or p.restart, rel_tol or p.rel_tol, max_iters or p.max_iters
     ref = oracle.gmres(p.A, p.b, p.x0, restart, rel_tol, max_iters, fmt, reorth=reorth)
@@ -35,7 +58,7 @@ def _check_parity(p, fmt, restart=None, rel_tol=None, max_iters=None, reorth="co
     true_gpu = _true_rel_res(p, x)
     true_ref = _true_rel_res(p, ref.x)
     assert r.converged == ref.converged
-    assert abs(r.iters - ref.iters) <= max(2, 0.02 * ref.iters), (fmt, r.iters, ref.iters)
+    _assert_iters_parity(r.iters, ref, p, fmt, restart, rel_tol, max_iters, reorth)
     if ref.converged:
         assert true_gpu <= rel_tol * (1 + 1e-9) and true_ref <= rel_tol * (1 + 1e-9)
     assert true_gpu <= 10 * true_ref and true_ref <= 10 * true_gpu
