@@ -131,11 +131,30 @@ const char *cbgmres_last_error(cbgmres_handle_t h);
 /* Tuning / test knobs, by name.  "spmv_kernel": 0 = choose from the row-length statistics,
  * L in {2,4,8,16,32} = L lanes per row, 64 = nnz-balanced streaming kernel.  "poll": 1 (default)
  * = the host stops launching a cycle's remaining steps once the device reports it left the cycle.
+ * "profile": 1 = time every kernel family with CUDA events (see cbgmres_profile_get), default 0.
  * Unknown names return CBGMRES_E_INVALID. */
 int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value);
 
 /* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
 int64_t cbgmres_launch_count(cbgmres_handle_t h);
+
+/* Per-kernel timing (option "profile" = 1): cbgmres_solve brackets every launch of the families
+ * below with CUDA events on its stream and accumulates, per family, the device time, the
+ * ALGORITHMIC bytes of those launches (S1 12 nnz + 4(n+1) + 16 n;
+ * S2 j n B + 8 n; S3 j n B + 16 n; S4 (16 + B) n; a fused S3+S2' launch counts j n B + 16 n)
+ * and their number.  Launches the device skipped (steps after the cycle's last, second passes that
+ * did not fire) are left out.  profile_get reads the totals since the last profile_reset. */
+#define CBGMRES_PROF_FAMILIES 6
+typedef enum {
+    CBGMRES_PROF_SPMV = 0,     /* S1 */
+    CBGMRES_PROF_MULTIDOT = 1, /* S2, S2' */
+    CBGMRES_PROF_UPDATE = 2,   /* S3, S3' */
+    CBGMRES_PROF_STORE = 3,    /* S4 (+ the Givens update riding on it) */
+    CBGMRES_PROF_XUPDATE = 4,  /* S6: back substitution + x += V y */
+    CBGMRES_PROF_RESIDUAL = 5  /* S7: r = b - A x and the store of v_1 */
+} cbgmres_prof_family_t;
+int cbgmres_profile_get(cbgmres_handle_t h, int32_t family, double *ms, double *bytes, int64_t *launches);
+int cbgmres_profile_reset(cbgmres_handle_t h);
 
 /* ---- per-kernel hooks (parity is judged per kernel: BASELINE.json north_star) ------------- */
 

@@ -6,6 +6,7 @@ from .binding import (  # noqa: F401
     FORMAT_CODE,
     EXPORTS,
     LIB_PATH,
+    PROF_FAMILIES,
     CbgmresError,
     Solver,
     SolveResult,

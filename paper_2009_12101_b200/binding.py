@@ -28,8 +28,9 @@ EXPORTS = (
     "cbgmres_create", "cbgmres_set_matrix", "cbgmres_workspace_bytes", "cbgmres_solve",
     "cbgmres_workspace_bytes_host", "cbgmres_solve_host", "cbgmres_destroy", "cbgmres_last_error",
     "cbgmres_set_option", "cbgmres_launch_count", "cbgmres_k_compress", "cbgmres_k_decode", "cbgmres_k_multidot",
-    "cbgmres_k_update", "cbgmres_k_store", "cbgmres_k_spmv",
+    "cbgmres_k_update", "cbgmres_k_store", "cbgmres_k_spmv", "cbgmres_profile_get", "cbgmres_profile_reset",
 )
+PROF_FAMILIES = ("spmv", "multidot", "update", "store", "xupdate", "residual")
 
 
 class Params(C.Structure):
@@ -81,6 +82,8 @@ def load_library(path: str = LIB_PATH):
     L.cbgmres_k_update.argtypes = [vp, i32, i64, i64, i32, vp, vp, vp, vp, vp, vp]
     L.cbgmres_k_store.argtypes = [vp, i32, i64, vp, dbl, dbl, vp, vp, vp]
     L.cbgmres_k_spmv.argtypes = [vp, vp, vp, vp]
+    L.cbgmres_profile_get.argtypes = [vp, i32, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i64)]
+    L.cbgmres_profile_reset.argtypes = [vp]
     for name in EXPORTS:
         if name not in ("cbgmres_last_error", "cbgmres_launch_count"):
             getattr(L, name).restype = C.c_int
@@ -164,6 +167,18 @@ class Solver:
 
     def launch_count(self) -> int:
         return int(self.lib.cbgmres_launch_count(self.h))
+
+    def profile_reset(self):
+        self._check(self.lib.cbgmres_profile_reset(self.h))
+
+    def profile_get(self) -> dict:
+        """{family: {"ms", "bytes", "launches"}} accumulated since profile_reset (option "profile" = 1)."""
+        out = {}
+        for i, name in enumerate(PROF_FAMILIES):
+            ms, by, cnt = C.c_double(0.0), C.c_double(0.0), C.c_int64(0)
+            self._check(self.lib.cbgmres_profile_get(self.h, i, C.byref(ms), C.byref(by), C.byref(cnt)))
+            out[name] = {"ms": ms.value, "bytes": by.value, "launches": int(cnt.value)}
+        return out
 
     def _dev(self, a, dtype):
         torch = _torch()

@@ -45,6 +45,7 @@ struct Ctl {
     int iters, max_iters, reorth_count, breakdown, converged, nonfinite, restarts, done;
     int reorth_mode, m, hist_cap;
     unsigned tickets[8]; // last-block-done counters, one per kernel family
+    unsigned char reorth_log[kMaxRestart + 8]; // reorth_flag of every step of the current cycle
 };
 
 // Small dense state of one restart cycle (device memory, < 3 MB at m = 512).

@@ -11,10 +11,21 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "internal.cuh"
 
 using namespace cbg;
+
+struct ProfSlot {
+    cudaEvent_t a = nullptr, b = nullptr;
+    int family = 0, step = 0, pass = 0;
+    double bytes = 0.0;
+};
+struct ProfAcc {
+    double ms = 0.0, bytes = 0.0;
+    int64_t launches = 0;
+};
 
 struct cbgmres_ctx {
     int device = 0;
@@ -33,6 +44,13 @@ struct cbgmres_ctx {
     int opt_poll = 1;
     int64_t launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    // optional per-kernel timing ("profile" option): event pairs around the launches of one cycle
+    int opt_profile = 0;
+    std::vector<ProfSlot> prof_slots;
+    int prof_used = 0;
+    int *h_reorth_log = nullptr; // mapped pinned [kMaxRestart + 2]: reorth_flag per step of the cycle
+    int *d_reorth_log = nullptr;
+    ProfAcc prof[CBGMRES_PROF_FAMILIES]{};
     char err[256] = "no error";
 };
 
@@ -120,6 +138,50 @@ int validate_params(cbgmres_ctx *h, const cbgmres_params *p)
     if (!(p->eta >= 0.0) || p->eta > 1.0) return fail(h, CBGMRES_E_INVALID, "eta must be in [0, 1]");
     if (p->res_history_cap < 0) return fail(h, CBGMRES_E_INVALID, "res_history_cap < 0");
     return CBGMRES_OK;
+}
+
+// ---- optional per-kernel timing ---------------------------------------------------------------
+// prof_begin/prof_end bracket one launch with an event pair; prof_collect runs after the cycle's
+// stream synchronisation, when the device's control block (k, reorth_log) is back on the host.
+void prof_begin(cbgmres_ctx *h, int family, int step, int pass, double bytes)
+{
+    if (!h->opt_profile) return;
+    if (h->prof_used == (int)h->prof_slots.size()) {
+        ProfSlot sl;
+        if (cudaEventCreate(&sl.a) != cudaSuccess || cudaEventCreate(&sl.b) != cudaSuccess) return;
+        h->prof_slots.push_back(sl);
+    }
+    ProfSlot &sl = h->prof_slots[h->prof_used];
+    sl.family = family;
+    sl.step = step;
+    sl.pass = pass;
+    sl.bytes = bytes;
+    cudaEventRecord(sl.a, h->stream);
+}
+
+void prof_end(cbgmres_ctx *h)
+{
+    if (!h->opt_profile || h->prof_used >= (int)h->prof_slots.size()) return;
+    cudaEventRecord(h->prof_slots[h->prof_used].b, h->stream);
+    h->prof_used += 1;
+}
+
+void prof_collect(cbgmres_ctx *h, const Ctl &c, bool cycle_ran)
+{
+    for (int i = 0; i < h->prof_used; ++i) {
+        const ProfSlot &sl = h->prof_slots[i];
+        bool ran = true;
+        if (sl.step > 0) ran = cycle_ran && sl.step <= c.k && (sl.pass < 2 || c.reorth_log[sl.step]);
+        else if (sl.family == CBGMRES_PROF_XUPDATE) ran = cycle_ran && c.k > 0;
+        if (!ran) continue;
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, sl.a, sl.b) != cudaSuccess) continue;
+        ProfAcc &acc = h->prof[sl.family];
+        acc.ms += ms;
+        acc.bytes += sl.bytes;
+        acc.launches += 1;
+    }
+    h->prof_used = 0;
 }
 
 int choose_spmv_kernel(cbgmres_ctx *h, int64_t n, int64_t nnz, int max_len)
@@ -224,6 +286,10 @@ int cbgmres_destroy(cbgmres_handle_t h)
     if (h->h_flag) cudaFreeHost(h->h_flag);
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
+    for (ProfSlot &sl : h->prof_slots) {
+        if (sl.a) cudaEventDestroy(sl.a);
+        if (sl.b) cudaEventDestroy(sl.b);
+    }
     delete h;
     return CBGMRES_OK;
 }
@@ -243,6 +309,10 @@ int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value)
     }
     if (!strcmp(name, "poll")) {
         h->opt_poll = value != 0;
+        return CBGMRES_OK;
+    }
+    if (!strcmp(name, "profile")) {
+        h->opt_profile = value != 0;
         return CBGMRES_OK;
     }
     return fail(h, CBGMRES_E_INVALID, "unknown option");
@@ -339,34 +409,64 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
     if (!std::isfinite(bnorm)) return fail(h, CBGMRES_E_NONFINITE, "||b|| is not finite");
 
     volatile int *flag = h->h_flag;
+    const double dn = (double)n, dB = (double)B;
+    const double bytes_spmv = 12.0 * (double)h->A.nnz + 4.0 * (dn + 1.0) + 16.0 * dn;
+    const double bytes_store = (16.0 + dB) * dn;
     for (;;) {
         *flag = INT_MAX;
+        h->prof_used = 0;
+        const int restarts_before = h->h_ctl->restarts;
         // l.1: r0 = b - A x, beta, the stopping test on the explicit residual; v1 = r0 / beta
+        prof_begin(h, CBGMRES_PROF_RESIDUAL, 0, 0, bytes_spmv + 8.0 * dn + bytes_store);
         h->launches += launch_spmv(s, h->sc, h->A, d_x, d_b, w, MODE_RESIDUAL, 0, &cy, h->d_flag);
         h->launches += launch_store(s, h->sc, fmt, n, w, &dctl->hn, &dctl->amax, 0.0, 0.0, Vp, cy.scales, v,
                                     MODE_RESIDUAL, 1, nullptr, nullptr);
+        prof_end(h);
         for (int j = 1; j <= m; ++j) {
             if (h->opt_poll && *flag < j) break; // the device already left this cycle
+            const double bytes_dot = (double)j * dn * dB + 8.0 * dn, bytes_upd = (double)j * dn * dB + 16.0 * dn;
             // l.3-4: w = A v, omega = ||w||
+            prof_begin(h, CBGMRES_PROF_SPMV, j, 0, bytes_spmv);
             h->launches += launch_spmv(s, h->sc, h->A, v, nullptr, w, MODE_STEP, j, nullptr, nullptr);
+            prof_end(h);
             // l.5-6: h = V^T w ; w -= V h ; h_{j+1,j} = ||w||
+            prof_begin(h, CBGMRES_PROF_MULTIDOT, j, 1, bytes_dot);
             h->launches += launch_multidot(s, h->sc, bv, n, j, w, cy.h, cy.hs, MODE_ORTH1, j);
+            prof_end(h);
+            prof_begin(h, CBGMRES_PROF_UPDATE, j, 1, bytes_upd);
             h->launches += launch_update(s, h->sc, bv, n, j, nullptr, cy.hs, w, MODE_ORTH1, j);
+            prof_end(h);
             if (p->reorth != CBGMRES_REORTH_NEVER) { // l.7-11, skipped on the device unless flagged
+                prof_begin(h, CBGMRES_PROF_MULTIDOT, j, 2, bytes_dot);
                 h->launches += launch_multidot(s, h->sc, bv, n, j, w, cy.h, cy.hs, MODE_ORTH2, j);
+                prof_end(h);
+                prof_begin(h, CBGMRES_PROF_UPDATE, j, 2, bytes_upd);
                 h->launches += launch_update(s, h->sc, bv, n, j, nullptr, cy.hs, w, MODE_ORTH2, j);
+                prof_end(h);
             }
             // l.13-14: v = w / h_{j+1,j}; V[:, j] = enc(v); + Givens update and stopping test
+            prof_begin(h, CBGMRES_PROF_STORE, j, 0, bytes_store);
             h->launches += launch_store(s, h->sc, fmt, n, w, &dctl->hn, &dctl->amax, 0.0, 0.0,
                                         Vp + (size_t)j * (size_t)L.ld * (size_t)B, cy.scales + j, v, MODE_ORTH1, j, &cy,
                                         h->d_flag);
+            prof_end(h);
         }
         // l.16-17: R y = g ; x += V_k y  (k read on the device)
+        prof_begin(h, CBGMRES_PROF_XUPDATE, 0, 0, 0.0);
         h->launches += launch_backsolve(s, h->sc, cy, fmt);
         h->launches += launch_update(s, h->sc, bv, n, 0, &dctl->k, cy.hs, d_x, MODE_XUPDATE, 0);
+        prof_end(h);
         CK(cudaMemcpyAsync(h->h_ctl, dctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
         CK(cudaStreamSynchronize(s));
         CK(cudaGetLastError());
+        if (h->opt_profile) {
+            const bool cycle_ran = h->h_ctl->restarts > restarts_before;
+            // the x update's bytes depend on k, known only now
+            for (int i = 0; i < h->prof_used; ++i)
+                if (h->prof_slots[i].family == CBGMRES_PROF_XUPDATE)
+                    h->prof_slots[i].bytes = (double)h->h_ctl->k * dn * dB + 16.0 * dn;
+            prof_collect(h, *h->h_ctl, cycle_ran);
+        }
         if (h->h_ctl->done) break;
     }
     if (hist_cap) {
@@ -440,6 +540,23 @@ int cbgmres_solve_host(cbgmres_handle_t h, int64_t n, int64_t nnz, const int32_t
     CK(cudaMemcpyAsync(h_x, d_x, (size_t)n * 8, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
     return rc;
+}
+
+int cbgmres_profile_get(cbgmres_handle_t h, int32_t family, double *ms, double *bytes, int64_t *launches)
+{
+    if (!h) return CBGMRES_E_INVALID;
+    if (family < 0 || family >= CBGMRES_PROF_FAMILIES) return fail(h, CBGMRES_E_INVALID, "unknown kernel family");
+    if (ms) *ms = h->prof[family].ms;
+    if (bytes) *bytes = h->prof[family].bytes;
+    if (launches) *launches = h->prof[family].launches;
+    return CBGMRES_OK;
+}
+
+int cbgmres_profile_reset(cbgmres_handle_t h)
+{
+    if (!h) return CBGMRES_E_INVALID;
+    for (ProfAcc &a : h->prof) a = ProfAcc{};
+    return CBGMRES_OK;
 }
 
 // ---- per-kernel hooks -------------------------------------------------------------------------------

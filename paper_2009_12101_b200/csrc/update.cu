@@ -155,6 +155,7 @@ __global__ void __launch_bounds__(THREADS) update_kernel(const UpdateArgs a)
                 ctl->breakdown = (hn == 0.0);
                 ctl->reorth_flag = (ctl->reorth_mode == CBGMRES_REORTH_ALWAYS) ||
                                    (ctl->reorth_mode == CBGMRES_REORTH_COND && hn < ctl->eta * ctl->omega);
+                ctl->reorth_log[a.step] = (unsigned char)ctl->reorth_flag;
                 if (!isfinite(hn)) ctl->nonfinite = 1;
             } else { // MODE_ORTH2, Fig. 1 l.10-12: new norm; breakdown if it again fell below eta * (norm before)
                 const double omega1 = ctl->hn;
