@@ -132,6 +132,9 @@ const char *cbgmres_last_error(cbgmres_handle_t h);
  * L in {2,4,8,16,32} = L lanes per row, 64 = nnz-balanced streaming kernel.  "poll": 1 (default)
  * = the host stops launching a cycle's remaining steps once the device reports it left the cycle.
  * "profile": 1 = time every kernel family with CUDA events (see cbgmres_profile_get), default 0.
+ * "orth_fuse": 1 (default) = fuse the first update with the second pass's multi-dot (one read of V).
+ * "orth_seg_kb": 0 (default, chosen per launch), 1, 2 or 4 = KB per column segment of the
+ * Gram-Schmidt passes' row tiles.
  * Unknown names return CBGMRES_E_INVALID. */
 int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value);
 
@@ -144,14 +147,15 @@ int64_t cbgmres_launch_count(cbgmres_handle_t h);
  * S2 j n B + 8 n; S3 j n B + 16 n; S4 (16 + B) n; a fused S3+S2' launch counts j n B + 16 n)
  * and their number.  Launches the device skipped (steps after the cycle's last, second passes that
  * did not fire) are left out.  profile_get reads the totals since the last profile_reset. */
-#define CBGMRES_PROF_FAMILIES 6
+#define CBGMRES_PROF_FAMILIES 7
 typedef enum {
     CBGMRES_PROF_SPMV = 0,     /* S1 */
     CBGMRES_PROF_MULTIDOT = 1, /* S2, S2' */
     CBGMRES_PROF_UPDATE = 2,   /* S3, S3' */
     CBGMRES_PROF_STORE = 3,    /* S4 (+ the Givens update riding on it) */
     CBGMRES_PROF_XUPDATE = 4,  /* S6: back substitution + x += V y */
-    CBGMRES_PROF_RESIDUAL = 5  /* S7: r = b - A x and the store of v_1 */
+    CBGMRES_PROF_RESIDUAL = 5, /* S7: r = b - A x and the store of v_1 */
+    CBGMRES_PROF_UPDATE_DOT = 6 /* S3 + S2' from one read of the basis */
 } cbgmres_prof_family_t;
 int cbgmres_profile_get(cbgmres_handle_t h, int32_t family, double *ms, double *bytes, int64_t *launches);
 int cbgmres_profile_reset(cbgmres_handle_t h);
@@ -172,6 +176,12 @@ int cbgmres_k_multidot(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld
  * *d_nrm2 <- ||w||_2 and *d_amax <- ||w||_inf of the new w, computed in the same pass. */
 int cbgmres_k_update(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld, int32_t k, const void *d_V,
                      const double *d_scales, const double *d_h, double *d_w, double *d_nrm2, double *d_amax);
+/* S3 + S2' fused, Fig. 1 lines 5-8: the update of k_update followed by
+ * d_u[c] <- sum_i dec(V)[i,c] * d_w_new[i], from one read of the basis.  k is limited by the
+ * shared-memory ring (128 at most; CBGMRES_E_INVALID beyond). */
+int cbgmres_k_update_multidot(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld, int32_t k, const void *d_V,
+                              const double *d_scales, const double *d_h, double *d_w, double *d_u, double *d_nrm2,
+                              double *d_amax);
 /* S4, Fig. 1 lines 13-14: d_v_fp64[i] <- d_w[i] / hnorm;
  * d_payload_col[n] <- enc(v); *d_scale <- sigma.  amax = ||w||_inf (only read by the integer formats). */
 int cbgmres_k_store(cbgmres_handle_t h, int32_t format, int64_t n, const double *d_w, double hnorm, double amax,

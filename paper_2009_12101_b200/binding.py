@@ -28,9 +28,9 @@ EXPORTS = (
     "cbgmres_create", "cbgmres_set_matrix", "cbgmres_workspace_bytes", "cbgmres_solve",
     "cbgmres_workspace_bytes_host", "cbgmres_solve_host", "cbgmres_destroy", "cbgmres_last_error",
     "cbgmres_set_option", "cbgmres_launch_count", "cbgmres_k_compress", "cbgmres_k_decode", "cbgmres_k_multidot",
-    "cbgmres_k_update", "cbgmres_k_store", "cbgmres_k_spmv", "cbgmres_profile_get", "cbgmres_profile_reset",
+    "cbgmres_k_update", "cbgmres_k_update_multidot", "cbgmres_k_store", "cbgmres_k_spmv", "cbgmres_profile_get", "cbgmres_profile_reset",
 )
-PROF_FAMILIES = ("spmv", "multidot", "update", "store", "xupdate", "residual")
+PROF_FAMILIES = ("spmv", "multidot", "update", "store", "xupdate", "residual", "update_multidot")
 
 
 class Params(C.Structure):
@@ -80,6 +80,7 @@ def load_library(path: str = LIB_PATH):
     L.cbgmres_k_decode.argtypes = [vp, i32, i64, vp, vp, vp]
     L.cbgmres_k_multidot.argtypes = [vp, i32, i64, i64, i32, vp, vp, vp, vp]
     L.cbgmres_k_update.argtypes = [vp, i32, i64, i64, i32, vp, vp, vp, vp, vp, vp]
+    L.cbgmres_k_update_multidot.argtypes = [vp, i32, i64, i64, i32, vp, vp, vp, vp, vp, vp, vp]
     L.cbgmres_k_store.argtypes = [vp, i32, i64, vp, dbl, dbl, vp, vp, vp]
     L.cbgmres_k_spmv.argtypes = [vp, vp, vp, vp]
     L.cbgmres_profile_get.argtypes = [vp, i32, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i64)]
@@ -297,6 +298,17 @@ class Solver:
                                               _ptr(scales), _ptr(h), _ptr(w), C.c_void_p(out.data_ptr()),
                                               C.c_void_p(out.data_ptr() + 8)))
         return out
+
+    def k_update_multidot(self, fmt: str, V, scales, h, w, n: int | None = None):
+        """Fused pass: w -= V h in place, then u = V^T w.  Returns (u, (nrm2, amax) device tensor)."""
+        torch = _torch()
+        n = w.numel() if n is None else n
+        out = torch.zeros(2, dtype=torch.float64, device=self.device)
+        u = torch.empty(h.numel(), dtype=torch.float64, device=self.device)
+        self._check(self.lib.cbgmres_k_update_multidot(self.h, FORMAT_CODE[fmt], n, V.shape[1], h.numel(), _ptr(V),
+                                                       _ptr(scales), _ptr(h), _ptr(w), _ptr(u),
+                                                       C.c_void_p(out.data_ptr()), C.c_void_p(out.data_ptr() + 8)))
+        return u, out
 
     def k_store(self, fmt: str, w, hnorm: float, amax: float, payload_col=None, v_out=None):
         torch = _torch()

@@ -44,6 +44,7 @@ struct Ctl {
     int k;            // Arnoldi steps completed in the current cycle
     int iters, max_iters, reorth_count, breakdown, converged, nonfinite, restarts, done;
     int reorth_mode, m, hist_cap;
+    int dir;          // row direction of the next Gram-Schmidt pass (flipped by every pass that runs)
     unsigned tickets[8]; // last-block-done counters, one per kernel family
     unsigned char reorth_log[kMaxRestart + 8]; // reorth_flag of every step of the current cycle
 };
@@ -83,10 +84,15 @@ struct CsrView {
 };
 
 // ---- launchers (each enqueues on `s` and returns the number of kernels launched) -------------
+// Gram-Schmidt passes (orth.cu).  seg_kb: 0 = choose the tile height, else 1, 2 or 4 KB per column segment.
 int launch_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t n, int k, const double *w,
-                    double *h_out, double *hs_out, int mode, int step);
+                    double *h_out, double *hs_out, int mode, int step, int seg_kb);
 int launch_update(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t n, int k, const int *d_k,
-                  const double *hs, double *w, int mode, int step);
+                  const double *hs, double *w, int mode, int step, int seg_kb);
+// fused update + next multi-dot; returns 0 (nothing launched) if k vectors do not fit the shared-memory ring
+int launch_update_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t n, int k, const double *hs,
+                           double *w, double *h_out, double *hs_out, int mode, int step, int seg_kb);
+bool update_multidot_fits(int format, int k, int seg_kb);
 int launch_store(cudaStream_t s, const Scratch &sc, int format, int64_t n, const double *w, const double *d_hn,
                  const double *d_amax, double hn_host, double amax_host, void *payload_col, double *scale_out,
                  double *v_out, int mode, int step, const CycleState *cyc, int *h_flag);

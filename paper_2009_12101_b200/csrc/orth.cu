@@ -1,0 +1,675 @@
+// orth.cu -- the Gram-Schmidt passes over the compressed basis (Fig. 1 lines 5-11 and 17,
+// PAPER.md:70-81, 92; the basis is read in its storage format and widened in registers,
+// PAPER.md:133, 169-181).  One persistent, TMA-fed kernel in three kinds:
+//
+//   PASS_DOT      h_c  = sum_i dec(V)[i,c] w_i                                  (S2,  l.5)
+//   PASS_UPD      w_i -= sum_c dec(V)[i,c] h_c, ||w||_2, ||w||_inf              (S3,  l.5-6 / l.8-10 / l.17)
+//   PASS_UPD_DOT  the update of the first Gram-Schmidt pass AND the inner products of the second
+//                 pass, u = dec(V)^T w_new, from ONE read of the basis          (S3 + S2', l.5-8)
+//
+// Bound: HBM.  Algorithmic bytes per launch: k n B + 8 n (DOT), k n B + 16 n (UPD, UPD_DOT).
+// Classical Gram-Schmidt with re-orthogonalisation reads V four times per Arnoldi step (dot, update,
+// dot, update); the fused middle pass makes that three, and consecutive passes walk the rows in
+// opposite directions so that the tail of one pass is still in the 126 MB L2 when the next begins.
+//
+// Mapping.  The n rows are cut into tiles of R rows, R*B = F KB per column segment (F = 1, 2, 4);
+// a tile is the sequence of column chunks [8 columns x R rows].  One persistent CTA per SM owns a
+// contiguous range of row tiles.  A producer warp streams chunks into a ring of shared-memory
+// stages (up to ~210 KB) with 1D bulk TMA copies (one copy per column segment, completion on an
+// mbarrier); sixteen consumer warps -- two row halves x eight columns -- work on a chunk as soon as
+// it lands: a warp owns one column of every chunk and one half of the rows, its lanes own 16-byte
+// payload words, so shared-memory reads are conflict free and every warp ends up with the CTA's
+// complete partial sums of ITS columns over its rows.  For the update each warp accumulates its
+// columns' contribution to its rows; the eight partial row vectors are added in a fixed order
+// through shared memory.  In PASS_UPD_DOT all chunks of a row tile stay resident until the new w
+// of that tile is known, then are swept a second time while the ring prefetches the next tile.
+// CTA partials go to global memory; the last CTA to finish adds them in a fixed order
+// (deterministic, no fp64 atomics), applies the per-vector scales and takes the decisions of
+// Fig. 1 lines 7 and 12 on the device.
+#include "device_utils.cuh"
+
+namespace cbg {
+
+enum PassKind : int { PASS_DOT = 0, PASS_UPD = 1, PASS_UPD_DOT = 2 };
+
+constexpr int kColWarps = 8;                            // columns per chunk: one per warp of a row half
+constexpr int kConsumerWarps = 2 * kColWarps;           // two row halves
+constexpr int kConsumers = kConsumerWarps * 32;
+constexpr int kOrthThreads = kConsumers + 32;           // + one producer warp
+constexpr int kChunkCols = kColWarps;
+constexpr int kMaxChunks = 16;                          // chunks per launch (accumulators live in registers)
+constexpr int kMaxRangeCols = kMaxChunks * kChunkCols;  // 128 columns per launch
+constexpr int kMaxStages = 32;
+constexpr int kOrthSmemBytes = 225 * 1024;              // dynamic shared memory of one CTA (one CTA per SM)
+
+struct OrthArgs {
+    const void *V;        // payload of the first column of this launch's range
+    int64_t ld;
+    const double *scales; // [k] sigma_c of the range (fixed-point formats)
+    const double *hs;     // [k] update coefficients sigma_c * h_c (UPD kinds)
+    const int *d_k;       // if non-null: total column count read on the device (cycle-end x update)
+    int c0;               //   ... and the first column of this launch's range within it
+    double *w;            // DOT: read; UPD kinds: read and written
+    int64_t n;
+    int k;                // columns of this launch (<= 128)
+    Ctl *ctl;
+    double *partials;     // [grid * kLdp]
+    double *npart;        // [2 * kMaxGrid]
+    double *h_out;        // DOT kinds: h (ORTH1: set; ORTH2 / fused: accumulated)
+    double *hs_out;       // DOT kinds: sigma_c * (h_c or u_c), the next update's coefficients
+    int mode, step;
+    int last_range;       // UPD kinds: the finaliser of this launch publishes the norms
+    int nstages, ntiles;
+};
+
+// ---- mbarrier / bulk-copy primitives (PTX) --------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LAB_DONE;\n"
+        "bra LAB_WAIT;\n"
+        "LAB_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+// 1D bulk copy global -> shared (TMA engine), bytes a multiple of 16, both addresses 16-byte aligned.
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void consumer_bar()
+{
+    asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory");
+}
+
+// ---- shared-memory map of one CTA -------------------------------------------------------------------
+//   [0, 1024)      mbarriers: full[32], empty[32], wfull[2], wempty[2]
+//   [1024, 2048)   hs_s[128]   update coefficients of this launch's columns
+//   [2048, 4096)   hpart[2][128] per-row-half dot partials of the CTA (epilogue)
+//   [4096, ...)    wbuf[2][R]  ring of w tiles
+//   then           red[8][R]   per-column-warp partial V h of the current tile (UPD kinds)
+//   then           stages[ns][8][SEG] ring of column chunks
+__host__ __device__ constexpr int orth_fixed_smem(int R, bool has_upd) { return 4096 + 16 * R + (has_upd ? 64 * R : 0); }
+
+template <int FMT, int F> struct Tile {
+    using Fm = Fmt<FMT>;
+    static constexpr int VEC = Fm::VEC, B = Fm::BYTES;
+    static constexpr int SEG = F * 1024;           // bytes of one column segment
+    static constexpr int R = SEG / B;              // rows of a tile
+    static constexpr int GV = F * VEC;             // rows (doubles) per lane and column
+    static constexpr int STAGE = kChunkCols * SEG; // bytes of one stage
+    static constexpr int WORDS_HALF = F * 32;      // 16-byte words per column and row half
+};
+
+// Decode the F payload words of this lane in column segment `seg` and hand VEC doubles per word to
+// `fn(f, d)`.  RAGGED: rows at or beyond `rows` are forced to zero (the payload there is stale
+// shared memory or padding and may decode to NaN).
+template <int FMT, int F, bool RAGGED, class Fn>
+__device__ __forceinline__ void for_words(const unsigned char *seg, int wi0, int rows, Fn &&fn)
+{
+    using T = Tile<FMT, F>;
+#pragma unroll
+    for (int f = 0; f < F; ++f) {
+        const int wi = wi0 + f * 32;
+        if (RAGGED && wi * T::VEC >= rows) continue;
+        const uint4 raw = *reinterpret_cast<const uint4 *>(seg + wi * 16);
+        double d[T::VEC];
+        T::Fm::decode(raw, d);
+        if (RAGGED) {
+#pragma unroll
+            for (int v = 0; v < T::VEC; ++v)
+                if (wi * T::VEC + v >= rows) d[v] = 0.0;
+        }
+        fn(f, d);
+    }
+}
+
+struct Ring {
+    int s = 0;
+    uint32_t ph = 0;
+    __device__ __forceinline__ void advance(int ns)
+    {
+        if (++s == ns) {
+            s = 0;
+            ph ^= 1u;
+        }
+    }
+};
+
+struct ConsumerCtx {
+    uint64_t *full, *empty, *wfull, *wempty;
+    const double *hs_s;
+    double *wbuf, *red;
+    unsigned char *stages;
+    int ns, k, nchunks;
+    int lane, cw, half, ct; // lane, column of the chunk, row half, consumer thread index
+};
+
+// One row tile on the consumer side.  acc[ch] are the lane's partial inner products of column
+// 8*ch + cw over its rows (kept across tiles); ss / am the lane's partial norms of the new w.
+template <int FMT, int F, int KIND, bool RAGGED>
+__device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArgs &a, int64_t r0, int rows, int wslot,
+                                             uint32_t wph, Ring &ring, double (&acc)[kMaxChunks], double &ss, double &am)
+{
+    using T = Tile<FMT, F>;
+    constexpr int VEC = T::VEC, GV = T::GV, R = T::R;
+    constexpr bool HAS_UPD = KIND != PASS_DOT, HAS_DOT = KIND != PASS_UPD;
+    const int wi0 = c.half * T::WORDS_HALF + c.lane; // this lane's first 16-byte word in a column segment
+    double *wt = c.wbuf + wslot * R;
+
+    mbar_wait(&c.wfull[wslot], wph);
+    if (RAGGED) { // rows beyond the tile's end read as zero; an odd last row is fetched by hand
+        if ((rows & 1) && c.ct == 0) wt[rows - 1] = a.w[r0 + rows - 1];
+        for (int r = rows + c.ct; r < R; r += kConsumers) wt[r] = 0.0;
+        consumer_bar();
+    }
+    auto load_w = [&](double (&wreg)[GV]) {
+#pragma unroll
+        for (int f = 0; f < F; ++f)
+#pragma unroll
+            for (int v = 0; v < VEC; v += 2) {
+                const double2 t = *reinterpret_cast<const double2 *>(wt + (wi0 + f * 32) * VEC + v);
+                wreg[f * VEC + v] = t.x;
+                wreg[f * VEC + v + 1] = t.y;
+            }
+    };
+    auto release_w = [&]() {
+        __syncwarp();
+        if (c.lane == 0) mbar_arrive(&c.wempty[wslot]);
+    };
+    auto release_stage = [&](int s) {
+        __syncwarp();
+        if (c.lane == 0) mbar_arrive(&c.empty[s]);
+    };
+
+    if (KIND == PASS_DOT) {
+        double wreg[GV];
+        load_w(wreg);
+        release_w();
+#pragma unroll
+        for (int ch = 0; ch < kMaxChunks; ++ch) {
+            if (ch < c.nchunks) {
+                mbar_wait(&c.full[ring.s], ring.ph);
+                if (ch * kChunkCols + c.cw < c.k) {
+                    const unsigned char *seg = c.stages + (size_t)ring.s * T::STAGE + c.cw * T::SEG;
+                    for_words<FMT, F, RAGGED>(seg, wi0, rows, [&](int f, const double(&d)[VEC]) {
+#pragma unroll
+                        for (int v = 0; v < VEC; ++v) acc[ch] = fma(d[v], wreg[f * VEC + v], acc[ch]);
+                    });
+                }
+                release_stage(ring.s);
+                ring.advance(c.ns);
+            }
+        }
+        return;
+    }
+
+    // ---- update: p = sum_c dec(V)[rows, c] * hs_c over this warp's columns -----------------------------
+    const Ring tile_start = ring;
+    double p[GV];
+#pragma unroll
+    for (int i = 0; i < GV; ++i) p[i] = 0.0;
+    for (int ch = 0; ch < c.nchunks; ++ch) {
+        mbar_wait(&c.full[ring.s], ring.ph);
+        const int col = ch * kChunkCols + c.cw;
+        if (col < c.k) {
+            const double coef = c.hs_s[col];
+            const unsigned char *seg = c.stages + (size_t)ring.s * T::STAGE + c.cw * T::SEG;
+            for_words<FMT, F, RAGGED>(seg, wi0, rows, [&](int f, const double(&d)[VEC]) {
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) p[f * VEC + v] = fma(d[v], coef, p[f * VEC + v]);
+            });
+        }
+        if (KIND == PASS_UPD) release_stage(ring.s);
+        ring.advance(c.ns);
+    }
+    double *redw = c.red + c.cw * R;
+#pragma unroll
+    for (int f = 0; f < F; ++f)
+#pragma unroll
+        for (int v = 0; v < VEC; v += 2)
+            *reinterpret_cast<double2 *>(redw + (wi0 + f * 32) * VEC + v) = make_double2(p[f * VEC + v], p[f * VEC + v + 1]);
+    consumer_bar();
+    // new w of the tile: the eight partial row vectors are added in a fixed order
+    for (int r = c.ct; r < R; r += kConsumers) {
+        double tot = 0.0;
+#pragma unroll
+        for (int q = 0; q < kColWarps; ++q) tot += c.red[q * R + r];
+        const double wn = wt[r] - tot;
+        if (!RAGGED || r < rows) {
+            a.w[r0 + r] = wn;
+            ss = fma(wn, wn, ss);
+            am = fmax(am, fabs(wn));
+            if (HAS_DOT) wt[r] = wn;
+        }
+    }
+    consumer_bar();
+    if (KIND == PASS_UPD) {
+        release_w();
+        return;
+    }
+
+    // ---- second sweep over the resident chunks: u_c += sum_rows dec(V)[r, c] * w_new[r] -----------------
+    double wreg[GV];
+    load_w(wreg);
+    fence_proxy_async(); // the slot was written through the generic proxy; the next writer is the TMA
+    release_w();
+    Ring r2 = tile_start;
+#pragma unroll
+    for (int ch = 0; ch < kMaxChunks; ++ch) {
+        if (ch < c.nchunks) {
+            if (ch * kChunkCols + c.cw < c.k) {
+                const unsigned char *seg = c.stages + (size_t)r2.s * T::STAGE + c.cw * T::SEG;
+                for_words<FMT, F, RAGGED>(seg, wi0, rows, [&](int f, const double(&d)[VEC]) {
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) acc[ch] = fma(d[v], wreg[f * VEC + v], acc[ch]);
+                });
+            }
+            release_stage(r2.s);
+            r2.advance(c.ns);
+        }
+    }
+    (void)HAS_UPD;
+}
+
+
+// ---- final stage, run by the CTA that finished last ---------------------------------------------------
+// Adds the CTA partials in a fixed order, applies the per-vector scales (h_c = sigma_c * sum q w),
+// and takes the decisions of Fig. 1 l.6-12 from the norms of the new w.
+template <int KIND, bool SCALED> __device__ void orth_finalize(const OrthArgs &a, int k, double *scratch)
+{
+    constexpr bool HAS_UPD = KIND != PASS_DOT, HAS_DOT = KIND != PASS_UPD;
+    constexpr int NW = kOrthThreads / 32;
+    Ctl *ctl = a.ctl;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nb = gridDim.x;
+    __shared__ int s_apply;
+    if (tid == 0) s_apply = 1;
+    __syncthreads();
+    if (HAS_UPD && a.last_range && warp == 0) {
+        double t = 0.0, m = 0.0;
+        for (int b = lane; b < nb; b += 32) {
+            t += __ldcg(&a.npart[b]);
+            m = fmax(m, __ldcg(&a.npart[kMaxGrid + b]));
+        }
+        t = warp_sum(t);
+        m = warp_max(m);
+        if (lane == 0) {
+            const double hn = sqrt(t);
+            if (a.mode == MODE_HOOK) {
+                ctl->hook_nrm2 = hn;
+                ctl->hook_amax = m;
+            } else if (a.mode == MODE_ORTH1) {
+                // Fig. 1 l.6-7: h_{j+1,j} := ||w||_2 ; re-orthogonalise iff h_{j+1,j} < eta * omega
+                const int flag = (ctl->reorth_mode == CBGMRES_REORTH_ALWAYS) ||
+                                 (ctl->reorth_mode == CBGMRES_REORTH_COND && hn < ctl->eta * ctl->omega);
+                ctl->hn = hn;
+                ctl->amax = m;
+                ctl->breakdown = (hn == 0.0);
+                ctl->reorth_flag = flag;
+                ctl->reorth_log[a.step] = (unsigned char)flag;
+                if (!isfinite(hn)) ctl->nonfinite = 1;
+                s_apply = flag;
+            } else if (a.mode == MODE_ORTH2) {
+                // Fig. 1 l.10-12: new norm; breakdown if it again fell below eta * (norm before the pass)
+                const double omega1 = ctl->hn;
+                ctl->hn = hn;
+                ctl->amax = m;
+                ctl->reorth_count += 1;
+                ctl->breakdown = (hn == 0.0) || (hn < ctl->eta * omega1);
+                if (!isfinite(hn)) ctl->nonfinite = 1;
+            }
+        }
+    }
+    __syncthreads();
+    if (HAS_DOT) {
+        double *part = scratch; // [NW][kMaxRangeCols]
+        for (int cg = 0; cg < k; cg += 32) {
+            const int col = cg + lane;
+            if (col < k) {
+                double sum = 0.0;
+                for (int b = warp; b < nb; b += NW) sum += __ldcg(&a.partials[(size_t)b * kLdp + col]);
+                part[warp * kMaxRangeCols + col] = sum;
+            }
+        }
+        __syncthreads();
+        const bool apply = s_apply != 0;
+        for (int col = tid; col < k; col += kOrthThreads) {
+            double tot = 0.0;
+#pragma unroll
+            for (int q = 0; q < NW; ++q) tot += part[q * kMaxRangeCols + col];
+            const double sigma = SCALED ? a.scales[col] : 1.0;
+            const double h = tot * sigma; // h_c = sigma_c * sum_i q_ic w_i
+            if (KIND == PASS_DOT) {
+                if (a.mode == MODE_ORTH2) a.h_out[col] += h; // Fig. 1 l.9: h_{1:j,j} += u
+                else a.h_out[col] = h;
+                if (a.hs_out) a.hs_out[col] = h * sigma;     // coefficient of the raw payload in the update
+            } else if (a.mode == MODE_HOOK) {
+                a.h_out[col] = h;
+                if (a.hs_out) a.hs_out[col] = h * sigma;
+            } else if (apply) { // fused pass inside the solver: u only counts if the second pass fires (l.7-9)
+                a.h_out[col] += h;
+                a.hs_out[col] = h * sigma;
+            }
+        }
+    }
+    if (a.mode != MODE_HOOK && a.last_range && tid == 0) ctl->dir ^= 1;
+}
+
+template <int FMT, int F, int KIND>
+__global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a)
+{
+    using T = Tile<FMT, F>;
+    constexpr int R = T::R, B = T::B;
+    constexpr bool HAS_UPD = KIND != PASS_DOT, HAS_DOT = KIND != PASS_UPD;
+    Ctl *ctl = a.ctl;
+    if (a.mode == MODE_ORTH1 || a.mode == MODE_ORTH2) {
+        if (a.step > ctl->stop_after) return;
+        if (a.mode == MODE_ORTH2 && !ctl->reorth_flag) return;
+    }
+    int k = a.k;
+    if (a.d_k) { // cycle-end x update: the number of basis vectors is only known on the device
+        k = min(a.k, *a.d_k - a.c0);
+        if (k <= 0) return;
+    }
+    const int nchunks = (k + kChunkCols - 1) / kChunkCols;
+    const int ns = a.nstages;
+
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem);
+    uint64_t *empty = full + kMaxStages;
+    uint64_t *wfull = empty + kMaxStages;
+    uint64_t *wempty = wfull + 2;
+    double *hs_s = reinterpret_cast<double *>(smem + 1024);
+    double *hpart = reinterpret_cast<double *>(smem + 2048);
+    double *wbuf = reinterpret_cast<double *>(smem + 4096);
+    double *red = wbuf + 2 * R;
+    unsigned char *stages = smem + orth_fixed_smem(R, HAS_UPD);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        for (int s = 0; s < ns; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], kConsumerWarps);
+        }
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(&wfull[s], 1);
+            mbar_init(&wempty[s], kConsumerWarps);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (HAS_UPD)
+        for (int c = tid; c < kMaxRangeCols; c += kOrthThreads) hs_s[c] = (c < k) ? a.hs[c] : 0.0;
+    __syncthreads();
+
+    // rows of this CTA: a contiguous range, a multiple of 64 rows (16-byte aligned in every format)
+    const int64_t per = ((a.n + gridDim.x - 1) / gridDim.x + 63) / 64 * 64;
+    const int64_t row_begin = min(a.n, (int64_t)blockIdx.x * per), row_end = min(a.n, row_begin + per);
+    const int ntiles = (int)((row_end - row_begin + R - 1) / R);
+    const int dir = (a.mode == MODE_HOOK) ? 0 : ctl->dir; // consecutive passes walk in opposite directions
+    const int64_t col_stride = a.ld * B;
+
+    double acc[kMaxChunks];
+#pragma unroll
+    for (int i = 0; i < kMaxChunks; ++i) acc[i] = 0.0;
+    double ss = 0.0, am = 0.0;
+
+    if (warp == kConsumerWarps) {
+        // ---- producer: one elected lane waits for free slots, lanes 0..7 issue one column copy each ----
+        Ring ring;
+        for (int i = 0; i < ntiles; ++i) {
+            const int t = dir ? ntiles - 1 - i : i;
+            const int64_t r0 = row_begin + (int64_t)t * R;
+            const int rows = (int)min((int64_t)R, row_end - r0);
+            const uint32_t seg_bytes = (uint32_t)((rows * B + 15) / 16 * 16);
+            const uint32_t w_bytes = (uint32_t)(rows * 8) & ~15u;
+            const int wslot = i & 1;
+            if (lane == 0) {
+                mbar_wait(&wempty[wslot], ((i >> 1) & 1) ^ 1u);
+                mbar_expect_tx(&wfull[wslot], w_bytes);
+                if (w_bytes) bulk_g2s(wbuf + wslot * R, a.w + r0, w_bytes, &wfull[wslot]);
+            }
+            const unsigned char *src = reinterpret_cast<const unsigned char *>(a.V) + r0 * B;
+            for (int ch = 0; ch < nchunks; ++ch) {
+                const int ncols = min(kChunkCols, k - ch * kChunkCols);
+                if (lane == 0) {
+                    mbar_wait(&empty[ring.s], ring.ph ^ 1u);
+                    mbar_expect_tx(&full[ring.s], ncols * seg_bytes);
+                }
+                __syncwarp();
+                if (lane < ncols)
+                    bulk_g2s(stages + (size_t)ring.s * T::STAGE + lane * T::SEG,
+                             src + (int64_t)(ch * kChunkCols + lane) * col_stride, seg_bytes, &full[ring.s]);
+                ring.advance(ns);
+            }
+        }
+    } else {
+        ConsumerCtx c{full, empty, wfull, wempty, hs_s, wbuf, red, stages, ns, k, nchunks, lane, warp & 7, warp >> 3, tid};
+        Ring ring;
+        for (int i = 0; i < ntiles; ++i) {
+            const int t = dir ? ntiles - 1 - i : i;
+            const int64_t r0 = row_begin + (int64_t)t * R;
+            const int rows = (int)min((int64_t)R, row_end - r0);
+            if (rows == R) consume_tile<FMT, F, KIND, false>(c, a, r0, rows, i & 1, (i >> 1) & 1, ring, acc, ss, am);
+            else consume_tile<FMT, F, KIND, true>(c, a, r0, rows, i & 1, (i >> 1) & 1, ring, acc, ss, am);
+        }
+        // ---- CTA partials ------------------------------------------------------------------------------
+        if (HAS_DOT) {
+            const double tot = butterfly_rec<kMaxChunks, 16>(acc, lane);
+            if (butterfly_owner<kMaxChunks>(lane)) {
+                const int col = butterfly_col<kMaxChunks>(lane) * kChunkCols + (warp & 7);
+                hpart[(warp >> 3) * kMaxRangeCols + col] = tot;
+            }
+        }
+        if (HAS_UPD) {
+            ss = warp_sum(ss);
+            am = warp_max(am);
+            if (lane == 0) {
+                red[warp] = ss;
+                red[kConsumerWarps + warp] = am;
+            }
+        }
+    }
+    __syncthreads();
+    if (HAS_DOT)
+        for (int col = tid; col < k; col += kOrthThreads)
+            a.partials[(size_t)blockIdx.x * kLdp + col] = hpart[col] + hpart[kMaxRangeCols + col];
+    if (HAS_UPD && tid == 0) {
+        double t = 0.0, m = 0.0;
+        for (int i = 0; i < kConsumerWarps; ++i) {
+            t += red[i];
+            m = fmax(m, red[kConsumerWarps + i]);
+        }
+        a.npart[blockIdx.x] = t;
+        a.npart[kMaxGrid + blockIdx.x] = m;
+    }
+    if (!last_block_done(&ctl->tickets[0])) return;
+    orth_finalize<KIND, T::Fm::SCALED>(a, k, reinterpret_cast<double *>(smem + 4096));
+}
+
+// ---- launchers ---------------------------------------------------------------------------------------
+namespace {
+
+inline int fmt_bytes(int format) { return format == CBGMRES_FP64 ? 8 : (format == CBGMRES_FP32 || format == CBGMRES_INT32) ? 4 : 2; }
+inline int fmt_max_seg_kb(int format) { return fmt_bytes(format) == 2 ? 2 : 4; } // F * VEC <= 16 rows per lane
+
+inline int stages_for(int format, int seg_kb, bool has_upd)
+{
+    const int R = seg_kb * 1024 / fmt_bytes(format);
+    const int ns = (kOrthSmemBytes - orth_fixed_smem(R, has_upd)) / (kChunkCols * seg_kb * 1024);
+    return ns > kMaxStages ? kMaxStages : ns;
+}
+
+// Column-segment size (KB) for a pass over k <= 128 columns; 0 = does not fit (fused kind only).
+// forced != 0 pins the size (clamped to what the format allows) when that is feasible.
+int choose_seg_kb(int format, int kind, int k, int64_t n, int forced)
+{
+    const int nchunks = (k + kChunkCols - 1) / kChunkCols;
+    const int B = fmt_bytes(format);
+    const int fmax = fmt_max_seg_kb(format);
+    const int64_t per = ((n + kNumSMs - 1) / kNumSMs + 63) / 64 * 64; // rows per CTA on a full grid
+    auto feasible = [&](int f) {
+        const int ns = stages_for(format, f, kind != PASS_DOT);
+        return kind == PASS_UPD_DOT ? ns >= nchunks + 1 : ns >= 3;
+    };
+    if (forced) {
+        const int f = forced > fmax ? fmax : forced;
+        if (feasible(f)) return f;
+    }
+    for (int f = fmax; f >= 1; f >>= 1) {
+        if (!feasible(f)) continue;
+        const int ns = stages_for(format, f, kind != PASS_DOT);
+        if (kind == PASS_UPD_DOT) { // room to prefetch the next row tile while this one is swept twice
+            const int want = nchunks + (nchunks / 2 > 4 ? nchunks / 2 : 4);
+            if (ns >= want || f == 1) return f;
+        } else if (f == 1 || (int64_t)f * 1024 / B * 2 <= per) { // at least two full tiles per CTA
+            return f;
+        }
+    }
+    return 0;
+}
+
+template <int FMT, int F, int KIND> int launch_inst(cudaStream_t s, OrthArgs &a)
+{
+    using T = Tile<FMT, F>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(orth_kernel<FMT, F, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, kOrthSmemBytes);
+        attr_set = true;
+    }
+    a.nstages = stages_for(FMT, F, KIND != PASS_DOT);
+    int64_t grid = (a.n + 63) / 64;
+    if (grid > kNumSMs) grid = kNumSMs;
+    const size_t smem = (size_t)orth_fixed_smem(T::R, KIND != PASS_DOT) + (size_t)a.nstages * T::STAGE;
+    orth_kernel<FMT, F, KIND><<<(int)grid, kOrthThreads, smem, s>>>(a);
+    return 1;
+}
+
+template <int FMT, int KIND> int launch_f(cudaStream_t s, OrthArgs &a, int seg_kb)
+{
+    constexpr int VEC = Fmt<FMT>::VEC;
+    switch (seg_kb) {
+    case 1: return launch_inst<FMT, 1, KIND>(s, a);
+    case 2: return launch_inst<FMT, 2, KIND>(s, a);
+    case 4:
+        if constexpr (VEC <= 4) return launch_inst<FMT, 4, KIND>(s, a);
+        return 0;
+    default: return 0;
+    }
+}
+
+template <int KIND> int launch_fmt(cudaStream_t s, int format, OrthArgs &a, int seg_kb)
+{
+    switch (format) {
+    case CBGMRES_FP64: return launch_f<CBGMRES_FP64, KIND>(s, a, seg_kb);
+    case CBGMRES_FP32: return launch_f<CBGMRES_FP32, KIND>(s, a, seg_kb);
+    case CBGMRES_FP16: return launch_f<CBGMRES_FP16, KIND>(s, a, seg_kb);
+    case CBGMRES_INT32: return launch_f<CBGMRES_INT32, KIND>(s, a, seg_kb);
+    case CBGMRES_INT16: return launch_f<CBGMRES_INT16, KIND>(s, a, seg_kb);
+    default: return 0;
+    }
+}
+
+OrthArgs base_args(const Scratch &sc, const BasisView &b, int64_t n, int mode, int step)
+{
+    OrthArgs a{};
+    a.V = b.V;
+    a.ld = b.ld;
+    a.scales = b.scales;
+    a.n = n;
+    a.ctl = sc.ctl;
+    a.partials = sc.partials;
+    a.npart = sc.npart;
+    a.mode = mode;
+    a.step = step;
+    a.last_range = 1;
+    return a;
+}
+
+} // namespace
+
+// S2 (and S2' when the fused pass does not fit): ranges of at most 128 columns per launch.
+int launch_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t n, int k, const double *w,
+                    double *h_out, double *hs_out, int mode, int step, int seg_kb)
+{
+    int launches = 0;
+    const int64_t col_bytes = b.ld * fmt_bytes(b.format);
+    for (int c0 = 0; c0 < k; c0 += kMaxRangeCols) {
+        const int kk = (k - c0 < kMaxRangeCols) ? k - c0 : kMaxRangeCols;
+        OrthArgs a = base_args(sc, b, n, mode, step);
+        a.V = static_cast<const char *>(b.V) + (int64_t)c0 * col_bytes;
+        a.scales = b.scales ? b.scales + c0 : nullptr;
+        a.w = const_cast<double *>(w);
+        a.k = kk;
+        a.h_out = h_out + c0;
+        a.hs_out = hs_out ? hs_out + c0 : nullptr;
+        a.last_range = (c0 + kMaxRangeCols >= k);
+        launches += launch_fmt<PASS_DOT>(s, b.format, a, choose_seg_kb(b.format, PASS_DOT, kk, n, seg_kb));
+    }
+    return launches;
+}
+
+// S3 / S3' / the x update of l.17 (d_k != null: the column count lives on the device, k is its bound).
+int launch_update(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t n, int k, const int *d_k,
+                  const double *hs, double *w, int mode, int step, int seg_kb)
+{
+    int launches = 0;
+    const int64_t col_bytes = b.ld * fmt_bytes(b.format);
+    for (int c0 = 0; c0 < k; c0 += kMaxRangeCols) {
+        const int kk = (k - c0 < kMaxRangeCols) ? k - c0 : kMaxRangeCols;
+        OrthArgs a = base_args(sc, b, n, mode, step);
+        a.V = static_cast<const char *>(b.V) + (int64_t)c0 * col_bytes;
+        a.hs = hs + c0;
+        a.d_k = d_k;
+        a.c0 = c0;
+        a.w = w;
+        a.k = kk;
+        a.last_range = (c0 + kMaxRangeCols >= k);
+        launches += launch_fmt<PASS_UPD>(s, b.format, a, choose_seg_kb(b.format, PASS_UPD, kk, n, seg_kb));
+    }
+    return launches;
+}
+
+bool update_multidot_fits(int format, int k, int seg_kb)
+{
+    return k >= 1 && k <= kMaxRangeCols && choose_seg_kb(format, PASS_UPD_DOT, k, 1 << 30, seg_kb) != 0;
+}
+
+int launch_update_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t n, int k, const double *hs,
+                           double *w, double *h_out, double *hs_out, int mode, int step, int seg_kb)
+{
+    if (!update_multidot_fits(b.format, k, seg_kb)) return 0;
+    OrthArgs a = base_args(sc, b, n, mode, step);
+    a.hs = hs;
+    a.w = w;
+    a.k = k;
+    a.h_out = h_out;
+    a.hs_out = hs_out;
+    return launch_fmt<PASS_UPD_DOT>(s, b.format, a, choose_seg_kb(b.format, PASS_UPD_DOT, k, n, seg_kb));
+}
+
+} // namespace cbg

@@ -42,6 +42,8 @@ struct cbgmres_ctx {
     int32_t *owned_blk_row = nullptr;
     int opt_spmv_kernel = 0;
     int opt_poll = 1;
+    int opt_seg_kb = 0; // column-segment size of the Gram-Schmidt passes (0 = auto)
+    int opt_fuse = 1;   // fused update + second-pass multi-dot
     int64_t launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     // optional per-kernel timing ("profile" option): event pairs around the launches of one cycle
@@ -311,6 +313,16 @@ int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value)
         h->opt_poll = value != 0;
         return CBGMRES_OK;
     }
+    if (!strcmp(name, "orth_seg_kb")) {
+        if (value != 0 && value != 1 && value != 2 && value != 4)
+            return fail(h, CBGMRES_E_INVALID, "orth_seg_kb must be 0, 1, 2 or 4");
+        h->opt_seg_kb = (int)value;
+        return CBGMRES_OK;
+    }
+    if (!strcmp(name, "orth_fuse")) {
+        h->opt_fuse = value != 0;
+        return CBGMRES_OK;
+    }
     if (!strcmp(name, "profile")) {
         h->opt_profile = value != 0;
         return CBGMRES_OK;
@@ -412,6 +424,7 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
     const double dn = (double)n, dB = (double)B;
     const double bytes_spmv = 12.0 * (double)h->A.nnz + 4.0 * (dn + 1.0) + 16.0 * dn;
     const double bytes_store = (16.0 + dB) * dn;
+    const int sk = h->opt_seg_kb;
     for (;;) {
         *flag = INT_MAX;
         h->prof_used = 0;
@@ -429,19 +442,34 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
             prof_begin(h, CBGMRES_PROF_SPMV, j, 0, bytes_spmv);
             h->launches += launch_spmv(s, h->sc, h->A, v, nullptr, w, MODE_STEP, j, nullptr, nullptr);
             prof_end(h);
-            // l.5-6: h = V^T w ; w -= V h ; h_{j+1,j} = ||w||
+            // l.5: h = V^T w
             prof_begin(h, CBGMRES_PROF_MULTIDOT, j, 1, bytes_dot);
-            h->launches += launch_multidot(s, h->sc, bv, n, j, w, cy.h, cy.hs, MODE_ORTH1, j);
+            h->launches += launch_multidot(s, h->sc, bv, n, j, w, cy.h, cy.hs, MODE_ORTH1, j, sk);
             prof_end(h);
-            prof_begin(h, CBGMRES_PROF_UPDATE, j, 1, bytes_upd);
-            h->launches += launch_update(s, h->sc, bv, n, j, nullptr, cy.hs, w, MODE_ORTH1, j);
-            prof_end(h);
-            if (p->reorth != CBGMRES_REORTH_NEVER) { // l.7-11, skipped on the device unless flagged
+            if (p->reorth == CBGMRES_REORTH_NEVER) {
+                // l.5-6: w -= V h ; h_{j+1,j} = ||w||
+                prof_begin(h, CBGMRES_PROF_UPDATE, j, 1, bytes_upd);
+                h->launches += launch_update(s, h->sc, bv, n, j, nullptr, cy.hs, w, MODE_ORTH1, j, sk);
+                prof_end(h);
+            } else if (h->opt_fuse && update_multidot_fits(fmt, j, sk)) {
+                // l.5-8 from one read of V: w -= V h, ||w||, and u = V^T w for the second pass;
+                // l.7 is decided on the device, u is dropped if the second pass does not fire
+                prof_begin(h, CBGMRES_PROF_UPDATE_DOT, j, 1, bytes_upd);
+                h->launches += launch_update_multidot(s, h->sc, bv, n, j, cy.hs, w, cy.h, cy.hs, MODE_ORTH1, j, sk);
+                prof_end(h);
+                // l.8-10: w -= V u ; h_{j+1,j} = ||w||   (skipped on the device unless flagged)
+                prof_begin(h, CBGMRES_PROF_UPDATE, j, 2, bytes_upd);
+                h->launches += launch_update(s, h->sc, bv, n, j, nullptr, cy.hs, w, MODE_ORTH2, j, sk);
+                prof_end(h);
+            } else {
+                prof_begin(h, CBGMRES_PROF_UPDATE, j, 1, bytes_upd);
+                h->launches += launch_update(s, h->sc, bv, n, j, nullptr, cy.hs, w, MODE_ORTH1, j, sk);
+                prof_end(h);
                 prof_begin(h, CBGMRES_PROF_MULTIDOT, j, 2, bytes_dot);
-                h->launches += launch_multidot(s, h->sc, bv, n, j, w, cy.h, cy.hs, MODE_ORTH2, j);
+                h->launches += launch_multidot(s, h->sc, bv, n, j, w, cy.h, cy.hs, MODE_ORTH2, j, sk);
                 prof_end(h);
                 prof_begin(h, CBGMRES_PROF_UPDATE, j, 2, bytes_upd);
-                h->launches += launch_update(s, h->sc, bv, n, j, nullptr, cy.hs, w, MODE_ORTH2, j);
+                h->launches += launch_update(s, h->sc, bv, n, j, nullptr, cy.hs, w, MODE_ORTH2, j, sk);
                 prof_end(h);
             }
             // l.13-14: v = w / h_{j+1,j}; V[:, j] = enc(v); + Givens update and stopping test
@@ -454,7 +482,7 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
         // l.16-17: R y = g ; x += V_k y  (k read on the device)
         prof_begin(h, CBGMRES_PROF_XUPDATE, 0, 0, 0.0);
         h->launches += launch_backsolve(s, h->sc, cy, fmt);
-        h->launches += launch_update(s, h->sc, bv, n, 0, &dctl->k, cy.hs, d_x, MODE_XUPDATE, 0);
+        h->launches += launch_update(s, h->sc, bv, n, m, &dctl->k, cy.hs, d_x, MODE_XUPDATE, 0, sk);
         prof_end(h);
         CK(cudaMemcpyAsync(h->h_ctl, dctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
         CK(cudaStreamSynchronize(s));
@@ -612,7 +640,7 @@ int cbgmres_k_multidot(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld
     if (k == 0) return CBGMRES_OK;
     CK(cudaSetDevice(h->device));
     BasisView bv{d_V, ld, d_scales, format};
-    h->launches += launch_multidot(h->stream, h->sc, bv, n, k, d_w, d_h, nullptr, MODE_HOOK, 0);
+    h->launches += launch_multidot(h->stream, h->sc, bv, n, k, d_w, d_h, nullptr, MODE_HOOK, 0, h->opt_seg_kb);
     CK(cudaGetLastError());
     return CBGMRES_OK;
 }
@@ -631,7 +659,32 @@ int cbgmres_k_update(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld, 
     CK(cudaSetDevice(h->device));
     BasisView bv{d_V, ld, d_scales, format};
     h->launches += launch_scale_coeffs(h->stream, k, d_h, scaled ? d_scales : nullptr, h->hook_hs);
-    h->launches += launch_update(h->stream, h->sc, bv, n, k, nullptr, h->hook_hs, d_w, MODE_HOOK, 0);
+    h->launches += launch_update(h->stream, h->sc, bv, n, k, nullptr, h->hook_hs, d_w, MODE_HOOK, 0, h->opt_seg_kb);
+    if (d_nrm2 || d_amax)
+        h->launches += launch_copy_scalars(h->stream, &h->sc.ctl->hook_nrm2, d_nrm2, &h->sc.ctl->hook_amax, d_amax);
+    CK(cudaGetLastError());
+    return CBGMRES_OK;
+}
+
+int cbgmres_k_update_multidot(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld, int32_t k, const void *d_V,
+                              const double *d_scales, const double *d_h, double *d_w, double *d_u, double *d_nrm2,
+                              double *d_amax)
+{
+    if (!h) return CBGMRES_E_INVALID;
+    const int rc = check_basis_args(h, format, n, ld, k, d_V);
+    if (rc) return rc;
+    if (!d_V || !d_w || !d_h || !d_u) return fail(h, CBGMRES_E_INVALID, "null pointer argument");
+    if (reinterpret_cast<uintptr_t>(d_w) % 16 != 0) return fail(h, CBGMRES_E_INVALID, "w must be 16-byte aligned");
+    const bool scaled = (format == CBGMRES_INT32 || format == CBGMRES_INT16);
+    if (scaled && !d_scales) return fail(h, CBGMRES_E_INVALID, "fixed-point formats need d_scales");
+    if (k == 0) return fail(h, CBGMRES_E_INVALID, "k must be >= 1");
+    if (!update_multidot_fits(format, k, h->opt_seg_kb))
+        return fail(h, CBGMRES_E_INVALID, "k vectors do not fit the fused pass (use k_update + k_multidot)");
+    CK(cudaSetDevice(h->device));
+    BasisView bv{d_V, ld, d_scales, format};
+    h->launches += launch_scale_coeffs(h->stream, k, d_h, scaled ? d_scales : nullptr, h->hook_hs);
+    h->launches += launch_update_multidot(h->stream, h->sc, bv, n, k, h->hook_hs, d_w, d_u, nullptr, MODE_HOOK, 0,
+                                          h->opt_seg_kb);
     if (d_nrm2 || d_amax)
         h->launches += launch_copy_scalars(h->stream, &h->sc.ctl->hook_nrm2, d_nrm2, &h->sc.ctl->hook_amax, d_amax);
     CK(cudaGetLastError());

@@ -49,11 +49,13 @@ def main(argv=None) -> int:
     ap.add_argument("--flush", action="store_true")
     ap.add_argument("--spmv", default="")
     ap.add_argument("--json", default="")
+    ap.add_argument("--seg-kb", type=int, default=0, help="orth_seg_kb option: 0 auto, 1, 2, 4")
     args = ap.parse_args(argv)
     ks = [int(x) for x in args.k.split(",") if x]
     fmts = [f for f in args.formats.split(",") if f]
     n, kmax = args.n, max(ks)
     s = Solver(0)
+    s.set_option("orth_seg_kb", args.seg_kb)
     dev = s.device
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev) if args.flush else None
     rows = []
@@ -77,6 +79,9 @@ def main(argv=None) -> int:
             hz = torch.zeros_like(h)  # w -= V*0 keeps w bounded over the repetitions; same traffic and flops
             med, best = _time(lambda: s.k_update(fmt, V[:k], sig, hz, w, n=n), args.reps, flush, torch)
             rows.append(("update", fmt, k, med, best, model.update_bytes(n, k, fmt)))
+            if k <= 128:
+                med, best = _time(lambda: s.k_update_multidot(fmt, V[:k], sig, hz, w, n=n), args.reps, flush, torch)
+                rows.append(("update_multidot", fmt, k, med, best, model.update_bytes(n, k, fmt)))
         col = torch.empty(ld, dtype=payload_dtype(fmt), device=dev)
         vout = torch.empty(n, dtype=torch.float64, device=dev)
         med, best = _time(lambda: s.k_store(fmt, w0, 2.0, 6.0, col, vout), args.reps, flush, torch)

@@ -153,6 +153,69 @@ def test_update_matches_oracle(solver, fmt, n, k):
 
 
 @pytest.mark.parametrize("fmt", FORMATS)
+@pytest.mark.parametrize("n,k", [(1, 1), (63, 3), (4096, 8), (50021, 9), (50021, 33), (200003, 100), (9473, 128)])
+def test_update_multidot_fused_matches_oracle(solver, fmt, n, k):
+    """S3 + S2' from one read of V: w_new = w - V^ h and u = V^^T w_new, against the oracle's
+    extended-precision update followed by its extended-precision multi-dot of the updated w."""
+    import torch
+
+    k = min(k, n)
+    P, sig, w, dP, dsig = _basis(fmt, n, k, seed=450 + n + k, ld_extra=64)
+    h = np.random.default_rng(451).standard_normal(k)
+    w_ref, ss_ref, am_ref = oracle.ref_update(fmt, P[:k], sig[:k], h, w)
+    u_ref = oracle.ref_multidot(fmt, P, sig, w_ref, k=k)
+    dw = _dev(w).clone()
+    u, out = solver.k_update_multidot(fmt, dP[:k], dsig[:k], _dev(h), dw, n=n)
+    torch.cuda.synchronize()
+    w_gpu, u_gpu = dw.cpu().numpy(), u.cpu().numpy()
+    nrm2, amax = out.cpu().numpy()
+    scale = np.linalg.norm(w) + np.linalg.norm(h)
+    Vhat_norm = np.array([np.linalg.norm(oracle.dec(fmt, P[c, :n], sig[c])) for c in range(k)])
+    assert np.linalg.norm(w_gpu - w_ref) <= TOL * scale
+    assert abs(nrm2 - np.sqrt(ss_ref)) <= TOL * scale
+    assert amax == np.abs(w_gpu).max()
+    assert np.all(np.isfinite(u_gpu))
+    # u inherits the update's error through V^^T: |du_c| <= ||v^_c|| ||dw|| + the dot's own rounding
+    assert np.all(np.abs(u_gpu - u_ref) <= 2 * TOL * Vhat_norm * scale)
+
+
+@pytest.mark.parametrize("fmt", FORMATS)
+@pytest.mark.parametrize("seg_kb", [1, 2, 4])
+@pytest.mark.parametrize("n,k", [(148 * 64 + 1, 5), (31111, 40), (70001, 129), (131072, 16)])
+def test_orth_passes_every_tile_height(fmt, seg_kb, n, k):
+    """Every column-segment size of the row tiles (1, 2, 4 KB), ragged tails, an odd n, more than
+    128 columns (two launches per pass)."""
+    import torch
+
+    from paper_2009_12101_b200 import Solver
+
+    s = Solver(0)
+    try:
+        s.set_option("orth_seg_kb", seg_kb)
+        P, sig, w, dP, dsig = _basis(fmt, n, k, seed=470 + n + k, ld_extra=64)
+        Vhat_norm = np.array([np.linalg.norm(oracle.dec(fmt, P[c, :n], sig[c])) for c in range(k)])
+        h_ref = oracle.ref_multidot(fmt, P, sig, w, k=k)
+        h = s.k_multidot(fmt, dP, dsig, _dev(w), n=n, k=k).cpu().numpy()
+        assert np.all(np.abs(h - h_ref) <= TOL * Vhat_norm * np.linalg.norm(w))
+        hh = np.random.default_rng(471).standard_normal(k)
+        w_ref, ss_ref, _ = oracle.ref_update(fmt, P[:k], sig[:k], hh, w)
+        dw = _dev(w).clone()
+        out = s.k_update(fmt, dP[:k], dsig[:k], _dev(hh), dw, n=n)
+        torch.cuda.synchronize()
+        scale = np.linalg.norm(w) + np.linalg.norm(hh)
+        assert np.linalg.norm(dw.cpu().numpy() - w_ref) <= TOL * scale
+        assert abs(out.cpu().numpy()[0] - np.sqrt(ss_ref)) <= TOL * scale
+        if k <= 128:
+            dw = _dev(w).clone()
+            u, out = s.k_update_multidot(fmt, dP[:k], dsig[:k], _dev(hh), dw, n=n)
+            u_ref = oracle.ref_multidot(fmt, P, sig, w_ref, k=k)
+            assert np.linalg.norm(dw.cpu().numpy() - w_ref) <= TOL * scale
+            assert np.all(np.abs(u.cpu().numpy() - u_ref) <= 2 * TOL * Vhat_norm * scale)
+    finally:
+        s.destroy()
+
+
+@pytest.mark.parametrize("fmt", FORMATS)
 def test_cgs_closed_form(solver, fmt):
     """w in span(V^): the dots return the coefficients and the update annihilates w."""
     n, k = 30011, 16
