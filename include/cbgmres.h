@@ -134,7 +134,8 @@ const char *cbgmres_last_error(cbgmres_handle_t h);
  * "profile": 1 = time every kernel family with CUDA events (see cbgmres_profile_get), default 0.
  * "orth_fuse": 1 (default) = fuse the first update with the second pass's multi-dot (one read of V).
  * "orth_seg_kb": 0 (default, chosen per launch), 1, 2 or 4 = KB per column segment of the
- * Gram-Schmidt passes' row tiles.
+ * Gram-Schmidt passes' row tiles.  "orth_interleave": 0 (default: short segments only), 1 = one
+ * contiguous row range per CTA, 2 = row tiles dealt round-robin to the CTAs (process-wide knob).
  * Unknown names return CBGMRES_E_INVALID. */
 int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value);
 

@@ -93,6 +93,8 @@ int launch_update(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t
 int launch_update_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t n, int k, const double *hs,
                            double *w, double *h_out, double *hs_out, int mode, int step, int seg_kb);
 bool update_multidot_fits(int format, int k, int seg_kb);
+int take_orth_error();           // CUresult of a failed tensor-map encode since the last call (0 = none)
+void set_orth_interleave(int v); // tuning knob: 0 auto, 1 blocked row ranges, 2 interleaved row tiles
 int launch_store(cudaStream_t s, const Scratch &sc, int format, int64_t n, const double *w, const double *d_hn,
                  const double *d_amax, double hn_host, double amax_host, void *payload_col, double *scale_out,
                  double *v_out, int mode, int step, const CycleState *cyc, int *h_flag);

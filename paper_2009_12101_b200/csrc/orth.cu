@@ -26,6 +26,8 @@
 // CTA partials go to global memory; the last CTA to finish adds them in a fixed order
 // (deterministic, no fp64 atomics), applies the per-vector scales and takes the decisions of
 // Fig. 1 lines 7 and 12 on the device.
+#include <cuda.h> // CUtensorMap (types only; the encoder is fetched with cudaGetDriverEntryPoint)
+
 #include "device_utils.cuh"
 
 namespace cbg {
@@ -39,7 +41,8 @@ constexpr int kOrthThreads = kConsumers + 32;           // + one producer warp
 constexpr int kChunkCols = kColWarps;
 constexpr int kMaxChunks = 16;                          // chunks per launch (accumulators live in registers)
 constexpr int kMaxRangeCols = kMaxChunks * kChunkCols;  // 128 columns per launch
-constexpr int kMaxStages = 32;
+constexpr int kMaxStages = 8;
+constexpr int kStageBytes = 32 * 1024;                  // 8 columns x 4 KB, 16 x 2 KB or 32 x 1 KB
 constexpr int kOrthSmemBytes = 225 * 1024;              // dynamic shared memory of one CTA (one CTA per SM)
 
 struct OrthArgs {
@@ -59,7 +62,8 @@ struct OrthArgs {
     double *hs_out;       // DOT kinds: sigma_c * (h_c or u_c), the next update's coefficients
     int mode, step;
     int last_range;       // UPD kinds: the finaliser of this launch publishes the norms
-    int nstages, ntiles;
+    int nstages;
+    int interleave;       // row tiles dealt round-robin to the CTAs (else one contiguous row range per CTA)
 };
 
 // ---- mbarrier / bulk-copy primitives (PTX) --------------------------------------------------------
@@ -98,6 +102,16 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src, uint32
                  "l"(src), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
 }
+// 2D tiled TMA copy global -> shared: box [box0 8-byte elements x 8 columns] at element (x, y) of
+// the basis seen as a 2D array of 8-byte words [columns][ld * B / 8]; out-of-range parts read as zero.
+__device__ __forceinline__ void tma_box_g2s(void *dst_smem, const CUtensorMap *map, int x, int y, uint64_t *bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+            smem_u32(dst_smem)),
+        "l"(map), "r"(x), "r"(y), "r"(smem_u32(bar))
+        : "memory");
+}
 __device__ __forceinline__ void fence_proxy_async()
 {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -122,22 +136,35 @@ template <int FMT, int F> struct Tile {
     static constexpr int SEG = F * 1024;           // bytes of one column segment
     static constexpr int R = SEG / B;              // rows of a tile
     static constexpr int GV = F * VEC;             // rows (doubles) per lane and column
-    static constexpr int STAGE = kChunkCols * SEG; // bytes of one stage
+    static constexpr int CPS = 4 / F;              // chunks per stage: a stage is always 32 columns-KB
+    static constexpr int STAGE_COLS = CPS * kChunkCols;
+    static constexpr int STAGE = STAGE_COLS * SEG; // bytes of one stage (32 KB)
     static constexpr int WORDS_HALF = F * 32;      // 16-byte words per column and row half
+    // TMA boxes: 8 columns x min(SEG, 2 KB); a stage is 4 (F = 1) or 2 (F = 2, 4) boxes.  For
+    // F = 4 the two boxes of a stage are the two 2 KB halves of the same 8 columns.
+    static constexpr int BOX_INNER = (F == 1 ? 1024 : 2048);
+    static constexpr int BOX_BYTES = kChunkCols * BOX_INNER;
+    static constexpr int BOXES = STAGE / BOX_BYTES;
+    // address of 16-byte word wi (0 .. SEG/16) of column lc (0 .. STAGE_COLS) of a stage
+    static __device__ __forceinline__ const unsigned char *word_ptr(const unsigned char *stage, int lc, int wi)
+    {
+        if constexpr (F == 4) return stage + (wi >> 7) * BOX_BYTES + lc * BOX_INNER + (wi & 127) * 16;
+        else return stage + lc * SEG + wi * 16;
+    }
 };
 
-// Decode the F payload words of this lane in column segment `seg` and hand VEC doubles per word to
+// Decode the F payload words of this lane in column `lc` of `stage` and hand VEC doubles per word to
 // `fn(f, d)`.  RAGGED: rows at or beyond `rows` are forced to zero (the payload there is stale
 // shared memory or padding and may decode to NaN).
 template <int FMT, int F, bool RAGGED, class Fn>
-__device__ __forceinline__ void for_words(const unsigned char *seg, int wi0, int rows, Fn &&fn)
+__device__ __forceinline__ void for_words(const unsigned char *stage, int lc, int wi0, int rows, Fn &&fn)
 {
     using T = Tile<FMT, F>;
 #pragma unroll
     for (int f = 0; f < F; ++f) {
         const int wi = wi0 + f * 32;
         if (RAGGED && wi * T::VEC >= rows) continue;
-        const uint4 raw = *reinterpret_cast<const uint4 *>(seg + wi * 16);
+        const uint4 raw = *reinterpret_cast<const uint4 *>(T::word_ptr(stage, lc, wi));
         double d[T::VEC];
         T::Fm::decode(raw, d);
         if (RAGGED) {
@@ -166,7 +193,7 @@ struct ConsumerCtx {
     const double *hs_s;
     double *wbuf, *red;
     unsigned char *stages;
-    int ns, k, nchunks;
+    int ns, k, nst; // ring size, columns of this launch, stages per row tile
     int lane, cw, half, ct; // lane, column of the chunk, row half, consumer thread index
 };
 
@@ -212,15 +239,20 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
         load_w(wreg);
         release_w();
 #pragma unroll
-        for (int ch = 0; ch < kMaxChunks; ++ch) {
-            if (ch < c.nchunks) {
+        for (int st = 0; st < kMaxChunks / T::CPS; ++st) {
+            if (st < c.nst) {
                 mbar_wait(&c.full[ring.s], ring.ph);
-                if (ch * kChunkCols + c.cw < c.k) {
-                    const unsigned char *seg = c.stages + (size_t)ring.s * T::STAGE + c.cw * T::SEG;
-                    for_words<FMT, F, RAGGED>(seg, wi0, rows, [&](int f, const double(&d)[VEC]) {
 #pragma unroll
-                        for (int v = 0; v < VEC; ++v) acc[ch] = fma(d[v], wreg[f * VEC + v], acc[ch]);
-                    });
+                for (int i = 0; i < T::CPS; ++i) {
+                    const int lc = i * kChunkCols + c.cw; // column within the stage
+                    if (st * T::STAGE_COLS + lc < c.k) {
+                        const unsigned char *stg = c.stages + (size_t)ring.s * T::STAGE;
+                        for_words<FMT, F, RAGGED>(stg, lc, wi0, rows, [&](int f, const double(&d)[VEC]) {
+#pragma unroll
+                            for (int v = 0; v < VEC; ++v)
+                                acc[st * T::CPS + i] = fma(d[v], wreg[f * VEC + v], acc[st * T::CPS + i]);
+                        });
+                    }
                 }
                 release_stage(ring.s);
                 ring.advance(c.ns);
@@ -234,16 +266,20 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
     double p[GV];
 #pragma unroll
     for (int i = 0; i < GV; ++i) p[i] = 0.0;
-    for (int ch = 0; ch < c.nchunks; ++ch) {
+    for (int st = 0; st < c.nst; ++st) {
         mbar_wait(&c.full[ring.s], ring.ph);
-        const int col = ch * kChunkCols + c.cw;
-        if (col < c.k) {
-            const double coef = c.hs_s[col];
-            const unsigned char *seg = c.stages + (size_t)ring.s * T::STAGE + c.cw * T::SEG;
-            for_words<FMT, F, RAGGED>(seg, wi0, rows, [&](int f, const double(&d)[VEC]) {
 #pragma unroll
-                for (int v = 0; v < VEC; ++v) p[f * VEC + v] = fma(d[v], coef, p[f * VEC + v]);
-            });
+        for (int i = 0; i < T::CPS; ++i) {
+            const int lc = i * kChunkCols + c.cw;
+            const int col = st * T::STAGE_COLS + lc;
+            if (col < c.k) {
+                const double coef = c.hs_s[col];
+                const unsigned char *stg = c.stages + (size_t)ring.s * T::STAGE;
+                for_words<FMT, F, RAGGED>(stg, lc, wi0, rows, [&](int f, const double(&d)[VEC]) {
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) p[f * VEC + v] = fma(d[v], coef, p[f * VEC + v]);
+                });
+            }
         }
         if (KIND == PASS_UPD) release_stage(ring.s);
         ring.advance(c.ns);
@@ -281,14 +317,19 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
     release_w();
     Ring r2 = tile_start;
 #pragma unroll
-    for (int ch = 0; ch < kMaxChunks; ++ch) {
-        if (ch < c.nchunks) {
-            if (ch * kChunkCols + c.cw < c.k) {
-                const unsigned char *seg = c.stages + (size_t)r2.s * T::STAGE + c.cw * T::SEG;
-                for_words<FMT, F, RAGGED>(seg, wi0, rows, [&](int f, const double(&d)[VEC]) {
+    for (int st = 0; st < kMaxChunks / T::CPS; ++st) {
+        if (st < c.nst) {
 #pragma unroll
-                    for (int v = 0; v < VEC; ++v) acc[ch] = fma(d[v], wreg[f * VEC + v], acc[ch]);
-                });
+            for (int i = 0; i < T::CPS; ++i) {
+                const int lc = i * kChunkCols + c.cw;
+                if (st * T::STAGE_COLS + lc < c.k) {
+                    const unsigned char *stg = c.stages + (size_t)r2.s * T::STAGE;
+                    for_words<FMT, F, RAGGED>(stg, lc, wi0, rows, [&](int f, const double(&d)[VEC]) {
+#pragma unroll
+                        for (int v = 0; v < VEC; ++v)
+                            acc[st * T::CPS + i] = fma(d[v], wreg[f * VEC + v], acc[st * T::CPS + i]);
+                    });
+                }
             }
             release_stage(r2.s);
             r2.advance(c.ns);
@@ -381,7 +422,7 @@ template <int KIND, bool SCALED> __device__ void orth_finalize(const OrthArgs &a
 }
 
 template <int FMT, int F, int KIND>
-__global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a)
+__global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a, const __grid_constant__ CUtensorMap tmap)
 {
     using T = Tile<FMT, F>;
     constexpr int R = T::R, B = T::B;
@@ -396,7 +437,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a)
         k = min(a.k, *a.d_k - a.c0);
         if (k <= 0) return;
     }
-    const int nchunks = (k + kChunkCols - 1) / kChunkCols;
+    const int nst = (k + T::STAGE_COLS - 1) / T::STAGE_COLS; // stages per row tile
     const int ns = a.nstages;
 
     extern __shared__ __align__(128) unsigned char smem[];
@@ -426,12 +467,27 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a)
         for (int c = tid; c < kMaxRangeCols; c += kOrthThreads) hs_s[c] = (c < k) ? a.hs[c] : 0.0;
     __syncthreads();
 
-    // rows of this CTA: a contiguous range, a multiple of 64 rows (16-byte aligned in every format)
-    const int64_t per = ((a.n + gridDim.x - 1) / gridDim.x + 63) / 64 * 64;
-    const int64_t row_begin = min(a.n, (int64_t)blockIdx.x * per), row_end = min(a.n, row_begin + per);
-    const int ntiles = (int)((row_end - row_begin + R - 1) / R);
+    // Row tiles of this CTA.  Blocked: one contiguous row range per CTA (a multiple of 64 rows, so
+    // every tile start is 16-byte aligned in every format), perfectly balanced whatever the tile
+    // height.  Interleaved: tile t belongs to CTA t mod grid, so the CTAs sweep a contiguous window
+    // of the basis together and short column segments still arrive at the DRAM as long runs.
+    int64_t row_begin, row_end, tile_stride;
+    int ntiles;
+    if (a.interleave) {
+        const int64_t total = (a.n + R - 1) / R;
+        ntiles = (int)((total - blockIdx.x + gridDim.x - 1) / gridDim.x);
+        if (ntiles < 0) ntiles = 0;
+        row_begin = (int64_t)blockIdx.x * R;
+        row_end = a.n;
+        tile_stride = (int64_t)gridDim.x * R;
+    } else {
+        const int64_t per = ((a.n + gridDim.x - 1) / gridDim.x + 63) / 64 * 64;
+        row_begin = min(a.n, (int64_t)blockIdx.x * per);
+        row_end = min(a.n, row_begin + per);
+        ntiles = (int)((row_end - row_begin + R - 1) / R);
+        tile_stride = R;
+    }
     const int dir = (a.mode == MODE_HOOK) ? 0 : ctl->dir; // consecutive passes walk in opposite directions
-    const int64_t col_stride = a.ld * B;
 
     double acc[kMaxChunks];
 #pragma unroll
@@ -443,9 +499,8 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a)
         Ring ring;
         for (int i = 0; i < ntiles; ++i) {
             const int t = dir ? ntiles - 1 - i : i;
-            const int64_t r0 = row_begin + (int64_t)t * R;
+            const int64_t r0 = row_begin + (int64_t)t * tile_stride;
             const int rows = (int)min((int64_t)R, row_end - r0);
-            const uint32_t seg_bytes = (uint32_t)((rows * B + 15) / 16 * 16);
             const uint32_t w_bytes = (uint32_t)(rows * 8) & ~15u;
             const int wslot = i & 1;
             if (lane == 0) {
@@ -453,26 +508,30 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a)
                 mbar_expect_tx(&wfull[wslot], w_bytes);
                 if (w_bytes) bulk_g2s(wbuf + wslot * R, a.w + r0, w_bytes, &wfull[wslot]);
             }
-            const unsigned char *src = reinterpret_cast<const unsigned char *>(a.V) + r0 * B;
-            for (int ch = 0; ch < nchunks; ++ch) {
-                const int ncols = min(kChunkCols, k - ch * kChunkCols);
+            const int x0 = (int)(r0 * B / 8); // first 8-byte word of the tile inside a column
+            for (int st = 0; st < nst; ++st) {
+                const int c_first = st * T::STAGE_COLS;
+                // boxes of this stage that hold at least one wanted column (F = 4: both halves of 8 columns)
+                const int nboxes = (F == 4) ? T::BOXES : min(T::BOXES, (k - c_first + kChunkCols - 1) / kChunkCols);
                 if (lane == 0) {
                     mbar_wait(&empty[ring.s], ring.ph ^ 1u);
-                    mbar_expect_tx(&full[ring.s], ncols * seg_bytes);
+                    mbar_expect_tx(&full[ring.s], nboxes * T::BOX_BYTES);
                 }
                 __syncwarp();
-                if (lane < ncols)
-                    bulk_g2s(stages + (size_t)ring.s * T::STAGE + lane * T::SEG,
-                             src + (int64_t)(ch * kChunkCols + lane) * col_stride, seg_bytes, &full[ring.s]);
+                if (lane < nboxes) {
+                    unsigned char *dst = stages + (size_t)ring.s * T::STAGE + lane * T::BOX_BYTES;
+                    if (F == 4) tma_box_g2s(dst, &tmap, x0 + lane * (T::BOX_INNER / 8), c_first, &full[ring.s]);
+                    else tma_box_g2s(dst, &tmap, x0, c_first + lane * kChunkCols, &full[ring.s]);
+                }
                 ring.advance(ns);
             }
         }
     } else {
-        ConsumerCtx c{full, empty, wfull, wempty, hs_s, wbuf, red, stages, ns, k, nchunks, lane, warp & 7, warp >> 3, tid};
+        ConsumerCtx c{full, empty, wfull, wempty, hs_s, wbuf, red, stages, ns, k, nst, lane, warp & 7, warp >> 3, tid};
         Ring ring;
         for (int i = 0; i < ntiles; ++i) {
             const int t = dir ? ntiles - 1 - i : i;
-            const int64_t r0 = row_begin + (int64_t)t * R;
+            const int64_t r0 = row_begin + (int64_t)t * tile_stride;
             const int rows = (int)min((int64_t)R, row_end - r0);
             if (rows == R) consume_tile<FMT, F, KIND, false>(c, a, r0, rows, i & 1, (i >> 1) & 1, ring, acc, ss, am);
             else consume_tile<FMT, F, KIND, true>(c, a, r0, rows, i & 1, (i >> 1) & 1, ring, acc, ss, am);
@@ -520,7 +579,7 @@ inline int fmt_max_seg_kb(int format) { return fmt_bytes(format) == 2 ? 2 : 4; }
 inline int stages_for(int format, int seg_kb, bool has_upd)
 {
     const int R = seg_kb * 1024 / fmt_bytes(format);
-    const int ns = (kOrthSmemBytes - orth_fixed_smem(R, has_upd)) / (kChunkCols * seg_kb * 1024);
+    const int ns = (kOrthSmemBytes - orth_fixed_smem(R, has_upd)) / kStageBytes;
     return ns > kMaxStages ? kMaxStages : ns;
 }
 
@@ -528,13 +587,13 @@ inline int stages_for(int format, int seg_kb, bool has_upd)
 // forced != 0 pins the size (clamped to what the format allows) when that is feasible.
 int choose_seg_kb(int format, int kind, int k, int64_t n, int forced)
 {
-    const int nchunks = (k + kChunkCols - 1) / kChunkCols;
     const int B = fmt_bytes(format);
     const int fmax = fmt_max_seg_kb(format);
     const int64_t per = ((n + kNumSMs - 1) / kNumSMs + 63) / 64 * 64; // rows per CTA on a full grid
+    auto tile_stages = [&](int f) { return (k * f + 31) / 32; };      // a stage holds 32 / f columns
     auto feasible = [&](int f) {
         const int ns = stages_for(format, f, kind != PASS_DOT);
-        return kind == PASS_UPD_DOT ? ns >= nchunks + 1 : ns >= 3;
+        return kind == PASS_UPD_DOT ? ns >= tile_stages(f) + 1 : ns >= 3;
     };
     if (forced) {
         const int f = forced > fmax ? fmax : forced;
@@ -542,30 +601,91 @@ int choose_seg_kb(int format, int kind, int k, int64_t n, int forced)
     }
     for (int f = fmax; f >= 1; f >>= 1) {
         if (!feasible(f)) continue;
-        const int ns = stages_for(format, f, kind != PASS_DOT);
-        if (kind == PASS_UPD_DOT) { // room to prefetch the next row tile while this one is swept twice
-            const int want = nchunks + (nchunks / 2 > 4 ? nchunks / 2 : 4);
-            if (ns >= want || f == 1) return f;
-        } else if (f == 1 || (int64_t)f * 1024 / B * 2 <= per) { // at least two full tiles per CTA
-            return f;
-        }
+        if (f == 1 || (int64_t)f * 1024 / B * 2 <= per) return f; // at least two full tiles per CTA
     }
     return 0;
+}
+
+int g_interleave_opt = 0; // 0 = interleave the short segments (1-2 KB), 1 = never, 2 = always
+int g_orth_error = 0;     // CUresult of the last failed tensor-map encode (0 = none)
+
+// ---- tensor maps: the basis as a 2D array [k columns][ceil(n*B/8) 8-byte words], box = 8 columns x
+// (1 or 2 KB).  Rows beyond n*B bytes and columns beyond k are out of range: not fetched, read as zero.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+struct MapKey {
+    const void *V = nullptr;
+    int64_t ld = 0, n = 0;
+    int bytes = 0, k = 0, inner = 0;
+    bool operator==(const MapKey &o) const
+    {
+        return V == o.V && ld == o.ld && n == o.n && bytes == o.bytes && k == o.k && inner == o.inner;
+    }
+};
+
+// One cached map per column count: inside a solve the same (V, k) comes back every restart cycle.
+const CUtensorMap *basis_map(const void *V, int64_t ld, int64_t n, int bytes, int k, int inner)
+{
+    struct Entry {
+        MapKey key;
+        CUtensorMap map;
+    };
+    static thread_local Entry cache[2][kMaxRangeCols + 1];
+    Entry &e = cache[inner == 1024 ? 0 : 1][k];
+    const MapKey key{V, ld, n, bytes, k, inner};
+    if (e.key == key) return &e.map;
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) {
+        g_orth_error = 999; // CUDA_ERROR_UNKNOWN: the driver has no cuTensorMapEncodeTiled
+        return nullptr;
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)((n * bytes + 7) / 8), (cuuint64_t)k};
+    const cuuint64_t strides[1] = {(cuuint64_t)(ld * bytes)};
+    const cuuint32_t box[2] = {(cuuint32_t)(inner / 8), (cuuint32_t)kChunkCols};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult rc = fn(&e.map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, const_cast<void *>(V), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (rc != CUDA_SUCCESS) {
+        g_orth_error = (int)rc;
+        e.key = MapKey{};
+        return nullptr;
+    }
+    e.key = key;
+    return &e.map;
 }
 
 template <int FMT, int F, int KIND> int launch_inst(cudaStream_t s, OrthArgs &a)
 {
     using T = Tile<FMT, F>;
+    a.interleave = g_interleave_opt == 2 || (g_interleave_opt == 0 && F <= 2);
     static bool attr_set = false;
     if (!attr_set) {
         cudaFuncSetAttribute(orth_kernel<FMT, F, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, kOrthSmemBytes);
         attr_set = true;
     }
+    const CUtensorMap *map = basis_map(a.V, a.ld, a.n, T::B, a.k, T::BOX_INNER);
+    if (!map) return 0;
     a.nstages = stages_for(FMT, F, KIND != PASS_DOT);
     int64_t grid = (a.n + 63) / 64;
     if (grid > kNumSMs) grid = kNumSMs;
     const size_t smem = (size_t)orth_fixed_smem(T::R, KIND != PASS_DOT) + (size_t)a.nstages * T::STAGE;
-    orth_kernel<FMT, F, KIND><<<(int)grid, kOrthThreads, smem, s>>>(a);
+    orth_kernel<FMT, F, KIND><<<(int)grid, kOrthThreads, smem, s>>>(a, *map);
     return 1;
 }
 
@@ -611,6 +731,14 @@ OrthArgs base_args(const Scratch &sc, const BasisView &b, int64_t n, int mode, i
 }
 
 } // namespace
+
+void set_orth_interleave(int v) { g_interleave_opt = v; }
+int take_orth_error()
+{
+    const int e = g_orth_error;
+    g_orth_error = 0;
+    return e;
+}
 
 // S2 (and S2' when the fused pass does not fit): ranges of at most 128 columns per launch.
 int launch_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t n, int k, const double *w,

@@ -319,6 +319,11 @@ int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value)
         h->opt_seg_kb = (int)value;
         return CBGMRES_OK;
     }
+    if (!strcmp(name, "orth_interleave")) {
+        if (value < 0 || value > 2) return fail(h, CBGMRES_E_INVALID, "orth_interleave must be 0, 1 or 2");
+        set_orth_interleave((int)value);
+        return CBGMRES_OK;
+    }
     if (!strcmp(name, "orth_fuse")) {
         h->opt_fuse = value != 0;
         return CBGMRES_OK;
@@ -487,6 +492,7 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
         CK(cudaMemcpyAsync(h->h_ctl, dctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
         CK(cudaStreamSynchronize(s));
         CK(cudaGetLastError());
+        if (take_orth_error()) return fail(h, CBGMRES_E_CUDA, "cuTensorMapEncodeTiled failed for the basis");
         if (h->opt_profile) {
             const bool cycle_ran = h->h_ctl->restarts > restarts_before;
             // the x update's bytes depend on k, known only now
@@ -641,6 +647,7 @@ int cbgmres_k_multidot(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld
     CK(cudaSetDevice(h->device));
     BasisView bv{d_V, ld, d_scales, format};
     h->launches += launch_multidot(h->stream, h->sc, bv, n, k, d_w, d_h, nullptr, MODE_HOOK, 0, h->opt_seg_kb);
+    if (take_orth_error()) return fail(h, CBGMRES_E_CUDA, "cuTensorMapEncodeTiled failed for the basis");
     CK(cudaGetLastError());
     return CBGMRES_OK;
 }
@@ -660,6 +667,7 @@ int cbgmres_k_update(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld, 
     BasisView bv{d_V, ld, d_scales, format};
     h->launches += launch_scale_coeffs(h->stream, k, d_h, scaled ? d_scales : nullptr, h->hook_hs);
     h->launches += launch_update(h->stream, h->sc, bv, n, k, nullptr, h->hook_hs, d_w, MODE_HOOK, 0, h->opt_seg_kb);
+    if (take_orth_error()) return fail(h, CBGMRES_E_CUDA, "cuTensorMapEncodeTiled failed for the basis");
     if (d_nrm2 || d_amax)
         h->launches += launch_copy_scalars(h->stream, &h->sc.ctl->hook_nrm2, d_nrm2, &h->sc.ctl->hook_amax, d_amax);
     CK(cudaGetLastError());
@@ -685,6 +693,7 @@ int cbgmres_k_update_multidot(cbgmres_handle_t h, int32_t format, int64_t n, int
     h->launches += launch_scale_coeffs(h->stream, k, d_h, scaled ? d_scales : nullptr, h->hook_hs);
     h->launches += launch_update_multidot(h->stream, h->sc, bv, n, k, h->hook_hs, d_w, d_u, nullptr, MODE_HOOK, 0,
                                           h->opt_seg_kb);
+    if (take_orth_error()) return fail(h, CBGMRES_E_CUDA, "cuTensorMapEncodeTiled failed for the basis");
     if (d_nrm2 || d_amax)
         h->launches += launch_copy_scalars(h->stream, &h->sc.ctl->hook_nrm2, d_nrm2, &h->sc.ctl->hook_amax, d_amax);
     CK(cudaGetLastError());

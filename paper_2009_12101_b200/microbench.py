@@ -49,6 +49,7 @@ def main(argv=None) -> int:
     ap.add_argument("--flush", action="store_true")
     ap.add_argument("--spmv", default="")
     ap.add_argument("--json", default="")
+    ap.add_argument("--interleave", type=int, default=0, help="orth_interleave option: 0 auto, 1 blocked, 2 interleaved")
     ap.add_argument("--seg-kb", type=int, default=0, help="orth_seg_kb option: 0 auto, 1, 2, 4")
     args = ap.parse_args(argv)
     ks = [int(x) for x in args.k.split(",") if x]
@@ -56,6 +57,7 @@ def main(argv=None) -> int:
     n, kmax = args.n, max(ks)
     s = Solver(0)
     s.set_option("orth_seg_kb", args.seg_kb)
+    s.set_option("orth_interleave", args.interleave)
     dev = s.device
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev) if args.flush else None
     rows = []
