@@ -78,8 +78,9 @@ struct CsrView {
     int64_t n, nnz;
     const int32_t *row_ptr, *col_idx;
     const double *vals;
-    const int32_t *blk_row; // [nblk+1] row partition of the streaming kernel (may be null)
+    const int4 *blk_desc;   // [nblk] row blocks of the streaming kernel {row0, row1, nz0, nz1} (may be null)
     int nblk;
+    int reduce_lanes;       // lanes sharing a row in the streaming kernel's row reduction (power of two)
     int kernel;             // 2,4,8,16,32 lanes per row, or 64 = streaming
 };
 
@@ -109,7 +110,7 @@ int launch_copy_scalars(cudaStream_t s, const double *src0, double *dst0, const 
 int launch_row_stats(cudaStream_t s, int64_t n, const int32_t *d_row_ptr, int *d_out);
 
 // row-partition metadata for the streaming SpMV (set_matrix)
-cudaError_t build_row_blocks(cudaStream_t s, int64_t n, int64_t nnz, const int32_t *d_row_ptr, int nnz_per_block,
-                             int32_t **d_blk_row_out, int *nblk_out);
+cudaError_t build_row_blocks(cudaStream_t s, int64_t n, int64_t nnz, const int32_t *d_row_ptr, int4 **d_desc_out,
+                             int *nblk_out);
 
 } // namespace cbg

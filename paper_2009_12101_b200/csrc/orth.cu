@@ -66,42 +66,6 @@ struct OrthArgs {
     int interleave;       // row tiles dealt round-robin to the CTAs (else one contiguous row range per CTA)
 };
 
-// ---- mbarrier / bulk-copy primitives (PTX) --------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra LAB_DONE;\n"
-        "bra LAB_WAIT;\n"
-        "LAB_DONE:\n"
-        "}\n" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-// 1D bulk copy global -> shared (TMA engine), bytes a multiple of 16, both addresses 16-byte aligned.
-__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(dst_smem)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
 // 2D tiled TMA copy global -> shared: box [box0 8-byte elements x 8 columns] at element (x, y) of
 // the basis seen as a 2D array of 8-byte words [columns][ld * B / 8]; out-of-range parts read as zero.
 __device__ __forceinline__ void tma_box_g2s(void *dst_smem, const CUtensorMap *map, int x, int y, uint64_t *bar)
@@ -175,18 +139,6 @@ __device__ __forceinline__ void for_words(const unsigned char *stage, int lc, in
         fn(f, d);
     }
 }
-
-struct Ring {
-    int s = 0;
-    uint32_t ph = 0;
-    __device__ __forceinline__ void advance(int ns)
-    {
-        if (++s == ns) {
-            s = 0;
-            ph ^= 1u;
-        }
-    }
-};
 
 struct ConsumerCtx {
     uint64_t *full, *empty, *wfull, *wempty;

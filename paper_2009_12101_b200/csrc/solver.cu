@@ -39,7 +39,7 @@ struct cbgmres_ctx {
     int *d_flag = nullptr;     // its device alias
     CsrView A{};
     bool has_matrix = false;
-    int32_t *owned_blk_row = nullptr;
+    int4 *owned_blk_row = nullptr;
     int opt_spmv_kernel = 0;
     int opt_poll = 1;
     int opt_seg_kb = 0; // column-segment size of the Gram-Schmidt passes (0 = auto)
@@ -190,13 +190,17 @@ int choose_spmv_kernel(cbgmres_ctx *h, int64_t n, int64_t nnz, int max_len)
 {
     if (h->opt_spmv_kernel) return h->opt_spmv_kernel;
     const double mean = n > 0 ? (double)nnz / (double)n : 0.0;
-    // irregular row lengths (power-law): stream nonzeros, reduce rows from shared memory
+    // irregular row lengths (power-law): stream nonzeros in storage order, reduce rows from shared memory
     if (max_len > 64 && (double)max_len > 8.0 * mean) return 64;
-    if (mean <= 3.0) return 2;
-    if (mean <= 6.0) return 4;
-    if (mean <= 12.0) return 8;
-    if (mean <= 40.0) return 16;
-    return 32;
+    // regular: row-major from shared memory; blocks of 256 RPT / LPR rows must hold <= 3584 nonzeros
+    const int len = (int)std::fmin((double)max_len, std::ceil(2.0 * mean));
+    if (len <= 3) return 132;  // 4 rows per thread
+    if (len <= 7) return 130;  // 2 rows per thread
+    if (len <= 14) return 129; // 1 row per thread
+    if (len <= 28) return 146; // 2 lanes per row
+    if (len <= 56) return 148; // 4 lanes per row
+    if (len <= 112) return 152; // 8 lanes per row
+    return 32;                 // a warp per row
 }
 
 int register_matrix(cbgmres_ctx *h, int64_t n, int64_t nnz, const int32_t *rp, const int32_t *ci, const double *va)
@@ -221,10 +225,12 @@ int register_matrix(cbgmres_ctx *h, int64_t n, int64_t nnz, const int32_t *rp, c
     h->A.kernel = choose_spmv_kernel(h, n, nnz, max_len);
     if (h->A.kernel == 64) {
         int nblk = 0;
-        CK(build_row_blocks(h->stream, n, nnz, rp, 0, &h->owned_blk_row, &nblk));
+        CK(build_row_blocks(h->stream, n, nnz, rp, &h->owned_blk_row, &nblk));
         h->launches += 1;
-        h->A.blk_row = h->owned_blk_row;
+        h->A.blk_desc = h->owned_blk_row;
         h->A.nblk = nblk;
+        const double mean = (double)nnz / (double)n; // about 4 products per lane
+        h->A.reduce_lanes = mean <= 6.0 ? 1 : mean <= 12.0 ? 2 : mean <= 24.0 ? 4 : mean <= 48.0 ? 8 : mean <= 96.0 ? 16 : 32;
     }
     h->has_matrix = true;
     return CBGMRES_OK;
@@ -304,8 +310,9 @@ int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value)
 {
     if (!h || !name) return CBGMRES_E_INVALID;
     if (!strcmp(name, "spmv_kernel")) {
-        if (value != 0 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32 && value != 64)
-            return fail(h, CBGMRES_E_INVALID, "spmv_kernel must be 0, 2, 4, 8, 16, 32 or 64");
+        if (value != 0 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32 && value != 64 &&
+            value != 129 && value != 130 && value != 132 && value != 146 && value != 148 && value != 152)
+            return fail(h, CBGMRES_E_INVALID, "spmv_kernel must be 0, 2, 4, 8, 16, 32, 64, 129, 130, 132, 146, 148 or 152");
         h->opt_spmv_kernel = (int)value;
         return CBGMRES_OK;
     }

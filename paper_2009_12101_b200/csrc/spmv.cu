@@ -113,7 +113,9 @@ __device__ __forceinline__ void block_norm_partials(const SpmvArgs &a, double ss
 }
 
 // ---- variant 1: LANES lanes per row ---------------------------------------------------------------
-template <int LANES> __global__ void __launch_bounds__(256) spmv_vec_kernel(const SpmvArgs a)
+// U rows per lane group are in flight at once: all row pointers first, then all (col, val) pairs,
+// then all gathers of x -- three rounds of independent loads instead of 3 U dependent ones.
+template <int LANES, int U> __global__ void __launch_bounds__(256) spmv_vec_kernel(const SpmvArgs a)
 {
     if (a.mode == MODE_STEP && a.step > a.ctl->stop_after) return;
     constexpr int RPB = 256 / LANES;
@@ -123,30 +125,91 @@ template <int LANES> __global__ void __launch_bounds__(256) spmv_vec_kernel(cons
     const double *__restrict__ va = a.A.vals;
     const double *__restrict__ x = a.x;
     double ss = 0.0, am = 0.0;
-    const int64_t nrows_pad = (a.A.n + RPB - 1) / RPB * RPB; // keep whole warps in the shuffles
-    for (int64_t row = (int64_t)blockIdx.x * RPB + sub; row < nrows_pad; row += (int64_t)gridDim.x * RPB) {
-        double s = 0.0;
-        if (row < a.A.n) {
-            const int p1 = rp[row + 1];
-            for (int p = rp[row] + sl; p < p1; p += LANES) s = fma(va[p], x[ci[p]], s);
+    const int64_t n = a.A.n;
+    const int64_t nrows_pad = (n + RPB - 1) / RPB * RPB; // keep whole warps in the shuffles
+    const int64_t stride = (int64_t)gridDim.x * RPB;
+    for (int64_t row0 = (int64_t)blockIdx.x * RPB + sub; row0 < nrows_pad; row0 += stride * U) {
+        int p[U], p1[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t row = row0 + u * stride;
+            p[u] = 0;
+            p1[u] = 0;
+            if (row < n) {
+                p[u] = rp[row] + sl;
+                p1[u] = rp[row + 1];
+            }
+        }
+        double s[U];
+        bool more = false;
+        int c[U];
+        double v[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) { // first LANES entries of every row: the whole row for short rows
+            s[u] = 0.0;
+            c[u] = 0;
+            v[u] = 0.0;
+            if (p[u] < p1[u]) {
+                c[u] = ci[p[u]];
+                v[u] = va[p[u]];
+            }
+            more |= p[u] + LANES < p1[u];
         }
 #pragma unroll
-        for (int o = LANES / 2; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        if (sl == 0 && row < a.A.n) {
-            const double val = (a.mode == MODE_RESIDUAL) ? a.b[row] - s : s;
-            a.w[row] = val;
-            ss = fma(val, val, ss);
-            am = fmax(am, fabs(val));
+        for (int u = 0; u < U; ++u) s[u] = v[u] * x[c[u]];
+        if (__any_sync(0xffffffffu, more)) {
+#pragma unroll
+            for (int u = 0; u < U; ++u)
+                for (int q = p[u] + LANES; q < p1[u]; q += LANES) s[u] = fma(va[q], x[ci[q]], s[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+#pragma unroll
+            for (int o = LANES / 2; o > 0; o >>= 1) s[u] += __shfl_xor_sync(0xffffffffu, s[u], o);
+            const int64_t row = row0 + u * stride;
+            if (sl == 0 && row < n) {
+                const double val = (a.mode == MODE_RESIDUAL) ? a.b[row] - s[u] : s[u];
+                a.w[row] = val;
+                ss = fma(val, val, ss);
+                am = fmax(am, fabs(val));
+            }
         }
     }
     block_norm_partials(a, ss, am, &a.ctl->tickets[2]);
 }
 
-// ---- variant 2: nnz-balanced streaming ---------------------------------------------------------------
-constexpr int kStreamT = 4096;      // target nonzeros per CTA (blocks are cut at multiples of T, whole rows)
-constexpr int kStreamBuf = 6000;    // product buffer: T + the overhang of the block's last row (static smem <= 48 KB)
+// ---- variant 2: nnz-balanced streaming (irregular row lengths) ------------------------------------------
+// A block is a run of whole rows holding about T nonzeros (descriptors made once in set_matrix).
+// Phase 1 streams the block's col_idx / vals with dense coalesced loads -- every thread first issues
+// ALL of its loads (T/256 index + value pairs, then as many gathers of x), so a CTA has ~T
+// independent requests in flight -- and leaves the products in shared memory.  Phase 2 reduces rows
+// from there (g lanes per row, a warp per very long row), in a fixed order.  The matrix is read once
+// per Arnoldi step and the basis passes stream hundreds of MB in between, so its lines are marked
+// evict-first in L2: the 126 MB L2 is kept for the basis and the vectors.
 constexpr int kStreamThreads = 256;
-constexpr int kLongRow = 64;        // rows longer than this are reduced by a whole warp
+constexpr int kStreamItems = 12;                          // nonzeros per thread and batch
+constexpr int kStreamT = kStreamThreads * kStreamItems;   // 3072 nonzeros per block
+constexpr int kStreamBuf = kStreamT + kStreamT / 2;       // + the overhang of the block's last row (36 KB)
+constexpr int kLongRow = 64;                              // rows longer than 64 g are reduced by a whole warp
+
+__device__ __forceinline__ uint64_t policy_evict_first()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ int ldg_stream_i32(const int32_t *p, uint64_t pol)
+{
+    int r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.b32 %0, [%1], %2;" : "=r"(r) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ double ldg_stream_f64(const double *p, uint64_t pol)
+{
+    double r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(r) : "l"(p), "l"(pol));
+    return r;
+}
 
 __global__ void __launch_bounds__(kStreamThreads) spmv_stream_kernel(const SpmvArgs a)
 {
@@ -156,42 +219,69 @@ __global__ void __launch_bounds__(kStreamThreads) spmv_stream_kernel(const SpmvA
     const int32_t *__restrict__ ci = a.A.col_idx;
     const double *__restrict__ va = a.A.vals;
     const double *__restrict__ x = a.x;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint64_t pol = policy_evict_first();
+    // g consecutive lanes share a row in phase 2 (a power of two <= 32 chosen from the mean row length):
+    // lane l of the group adds products l, l+g, ... and a butterfly adds the g partial sums.
+    const int g = a.A.reduce_lanes, gl = tid & (g - 1), rows_per_pass = kStreamThreads / g;
     double ss = 0.0, am = 0.0;
     for (int blk = blockIdx.x; blk < a.A.nblk; blk += gridDim.x) {
-        const int r0 = a.A.blk_row[blk], r1 = a.A.blk_row[blk + 1];
+        const int4 d = a.A.blk_desc[blk]; // {first row, end row, first nonzero, end nonzero}
+        const int r0 = d.x, r1 = d.y, p0 = d.z, cnt = d.w - d.z;
         if (r0 >= r1) continue;
-        const int p0 = rp[r0], p1 = rp[r1];
-        if (p1 - p0 <= kStreamBuf) {
+        if (cnt <= kStreamBuf) {
+            __syncthreads(); // the previous block's phase 2 has finished with prod[]
+            for (int off = 0; off < cnt; off += kStreamT) {
+                int c[kStreamItems];
+                double v[kStreamItems];
+#pragma unroll
+                for (int i = 0; i < kStreamItems; ++i) {
+                    const int q = off + i * kStreamThreads + tid;
+                    c[i] = 0;
+                    v[i] = 0.0;
+                    if (q < cnt) {
+                        c[i] = ldg_stream_i32(ci + p0 + q, pol);
+                        v[i] = ldg_stream_f64(va + p0 + q, pol);
+                    }
+                }
+                double xv[kStreamItems];
+#pragma unroll
+                for (int i = 0; i < kStreamItems; ++i) xv[i] = __ldg(x + c[i]);
+#pragma unroll
+                for (int i = 0; i < kStreamItems; ++i) {
+                    const int q = off + i * kStreamThreads + tid;
+                    if (q < cnt) prod[q] = v[i] * xv[i];
+                }
+            }
             __syncthreads();
-            for (int p = p0 + threadIdx.x; p < p1; p += kStreamThreads) prod[p - p0] = va[p] * x[ci[p]];
-            __syncthreads();
-            // short rows: one thread each, sequential over the row's products; a long row is reduced
-            // by the whole warp that found it (ballot), so the order of every sum is fixed
-            for (int rb = r0; rb < r1; rb += kStreamThreads) {
-                const int r = rb + threadIdx.x;
+            for (int rb = r0; rb < r1; rb += rows_per_pass) {
+                const int r = rb + tid / g;
                 const bool valid = r < r1;
-                const int q0 = valid ? rp[r] - p0 : 0, q1 = valid ? rp[r + 1] - p0 : 0;
-                const bool is_long = (q1 - q0) > kLongRow;
-                if (valid && !is_long) {
-                    double s = 0.0;
-                    for (int q = q0; q < q1; ++q) s += prod[q];
-                    const double val = (a.mode == MODE_RESIDUAL) ? a.b[r] - s : s;
+                const int a0 = valid ? rp[r] - p0 : 0, a1 = valid ? rp[r + 1] - p0 : 0;
+                const double bv = (valid && a.mode == MODE_RESIDUAL) ? a.b[r] : 0.0;
+                const bool is_long = valid && (a1 - a0) > kLongRow * g;
+                double s = 0.0;
+                if (valid && !is_long)
+                    for (int q = a0 + gl; q < a1; q += g) s += prod[q];
+                for (int o = g >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+                if (valid && !is_long && gl == 0) {
+                    const double val = (a.mode == MODE_RESIDUAL) ? bv - s : s;
                     a.w[r] = val;
                     ss = fma(val, val, ss);
                     am = fmax(am, fabs(val));
                 }
-                unsigned mask = __ballot_sync(0xffffffffu, is_long);
-                while (mask) {
+                unsigned mask = __ballot_sync(0xffffffffu, is_long && gl == 0);
+                while (mask) { // a very long row is reduced by the whole warp that found it: fixed order
                     const int src = __ffs(mask) - 1;
                     mask &= mask - 1;
-                    const int rr = rb + warp * 32 + src;
-                    const int qq0 = __shfl_sync(0xffffffffu, q0, src), qq1 = __shfl_sync(0xffffffffu, q1, src);
-                    double s = 0.0;
-                    for (int q = qq0 + lane; q < qq1; q += 32) s += prod[q];
-                    s = warp_sum(s);
+                    const int rr = __shfl_sync(0xffffffffu, r, src);
+                    const int qq0 = __shfl_sync(0xffffffffu, a0, src), qq1 = __shfl_sync(0xffffffffu, a1, src);
+                    const double bb = __shfl_sync(0xffffffffu, bv, src);
+                    double t = 0.0;
+                    for (int q = qq0 + lane; q < qq1; q += 32) t += prod[q];
+                    t = warp_sum(t);
                     if (lane == 0) {
-                        const double val = (a.mode == MODE_RESIDUAL) ? a.b[rr] - s : s;
+                        const double val = (a.mode == MODE_RESIDUAL) ? bb - t : t;
                         a.w[rr] = val;
                         ss = fma(val, val, ss);
                         am = fmax(am, fabs(val));
@@ -217,36 +307,221 @@ __global__ void __launch_bounds__(kStreamThreads) spmv_stream_kernel(const SpmvA
     block_norm_partials(a, ss, am, &a.ctl->tickets[2]);
 }
 
-// Row partition of the streaming kernel: blk_row[b] = first row r with row_ptr[r] >= b*T, so block b
-// holds whole rows and about T nonzeros.
-__global__ void row_blocks_kernel(int64_t n, const int32_t *__restrict__ rp, int T, int nblk, int32_t *blk_row)
+// ---- variant 3: row-major from shared memory (regular matrices: stencils, banded, FEM) --------------
+// Blocks of RB = 256 RPT / LPR consecutive rows, sized so that a block's nonzeros fit a stage:
+// RPT rows per thread (short rows) or LPR lanes per row (long rows), at most ~14 nonzeros per thread.
+// Two persistent CTAs per SM; a producer warp streams each block's col_idx / vals / row pointers
+// into a two-stage shared-memory ring with bulk TMA copies (up to 43 KB per stage).  The consumer
+// threads walk their rows in CSR order straight from shared memory, so the 32 lanes of a warp read
+// THE SAME DIAGONALS of consecutive rows and the gathers of x coalesce into a few 128-byte lines --
+// instead of the 8-16 lines a warp touches when it walks the nonzeros in storage order.  All of a
+// thread's gathers (16) are issued before the first is used: one exposed latency per block.
+// No CTA barrier: warps only meet at the mbarriers.
+constexpr int kRowsThreads = 256;
+constexpr int kRowsCta = kRowsThreads + 32;
+constexpr int kRowsBuf = 3584;  // nonzeros per stage (256 threads x 14)
+constexpr int kRowsMaxRows = 1024;
+constexpr int kRowsStages = 2;
+constexpr int kRowsGathers = 16; // gathers in flight per thread and round
+
+struct RowsStage {
+    int32_t ci[kRowsBuf + 4];
+    int32_t rp[kRowsMaxRows + 8];
+    double va[kRowsBuf + 2];
+};
+struct RowsSmem {
+    uint64_t full[kRowsStages], empty[kRowsStages];
+    RowsStage st[kRowsStages];
+};
+
+template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_rows_kernel(const SpmvArgs a)
 {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b > nblk) return;
-    if (b == nblk) {
-        blk_row[b] = (int32_t)n;
-        return;
+    if (a.mode == MODE_STEP && a.step > a.ctl->stop_after) return;
+    constexpr int RB = kRowsThreads * RPT / LPR, KU = kRowsGathers / RPT, RSTRIDE = kRowsThreads / LPR;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    RowsSmem &sm = *reinterpret_cast<RowsSmem *>(smem_raw);
+    const int32_t *__restrict__ rp = a.A.row_ptr;
+    const int32_t *__restrict__ ci = a.A.col_idx;
+    const double *__restrict__ va = a.A.vals;
+    const double *__restrict__ x = a.x;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int n = (int)a.A.n;
+    const int safe_ci = (int)(a.A.nnz & ~(int64_t)3), safe_va = (int)(a.A.nnz & ~(int64_t)1);
+    const int safe_rp = (int)((a.A.n + 1) & ~(int64_t)3);
+    if (tid == 0) {
+        for (int s = 0; s < kRowsStages; ++s) {
+            mbar_init(&sm.full[s], 1);
+            mbar_init(&sm.empty[s], kRowsThreads / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    const int64_t target = (int64_t)b * T;
-    int64_t lo = 0, hi = n; // first r in [0, n] with rp[r] >= target
-    while (lo < hi) {
-        const int64_t mid = (lo + hi) >> 1;
-        if (rp[mid] >= target) hi = mid;
-        else lo = mid + 1;
+    __syncthreads();
+    double ss = 0.0, am = 0.0;
+    const int nblk = (n + RB - 1) / RB, stride = gridDim.x;
+
+    if (warp == kRowsThreads / 32) {
+        // ---- producer ----------------------------------------------------------------------------------
+        Ring ring;
+        int np0 = 0, np1 = 0;
+        if ((int)blockIdx.x < nblk) {
+            np0 = rp[blockIdx.x * RB];
+            np1 = rp[min(n, (int)(blockIdx.x + 1) * RB)];
+        }
+        for (int blk = blockIdx.x; blk < nblk; blk += stride) {
+            const int r0 = blk * RB, r1 = min(n, r0 + RB), p0 = np0, p1 = np1;
+            if (blk + stride < nblk) { // row pointers of the next block, one iteration ahead
+                np0 = rp[(blk + stride) * RB];
+                np1 = rp[min(n, (blk + stride + 1) * RB)];
+            }
+            if (lane == 0) {
+                mbar_wait(&sm.empty[ring.s], ring.ph ^ 1u);
+                RowsStage &st = sm.st[ring.s];
+                uint32_t bytes_ci = 0, bytes_va = 0, bytes_rp = 0;
+                const int pc = p0 & ~3, pv = p0 & ~1, ra = r0 & ~3;
+                bytes_rp = (uint32_t)max(0, min((r1 + 1 + 3) & ~3, safe_rp) - ra) * 4u;
+                if (p1 - p0 <= kRowsBuf) { // else: the consumers take this block straight from global memory
+                    bytes_ci = (uint32_t)max(0, min((p1 + 3) & ~3, safe_ci) - pc) * 4u;
+                    bytes_va = (uint32_t)max(0, min((p1 + 1) & ~1, safe_va) - pv) * 8u;
+                }
+                mbar_expect_tx(&sm.full[ring.s], bytes_ci + bytes_va + bytes_rp);
+                if (bytes_ci) bulk_g2s(st.ci, ci + pc, bytes_ci, &sm.full[ring.s]);
+                if (bytes_va) bulk_g2s(st.va, va + pv, bytes_va, &sm.full[ring.s]);
+                if (bytes_rp) bulk_g2s(st.rp, rp + ra, bytes_rp, &sm.full[ring.s]);
+            }
+            __syncwarp();
+            ring.advance(kRowsStages);
+        }
+    } else {
+        // ---- consumers: lane group tid / LPR owns rows r0 + tid / LPR + u * RSTRIDE of the block ----------
+        const int gl = tid % LPR;
+        Ring ring;
+        for (int blk = blockIdx.x; blk < nblk; blk += stride) {
+            const int r0 = blk * RB, r1 = min(n, r0 + RB), ra = r0 & ~3;
+            mbar_wait(&sm.full[ring.s], ring.ph);
+            const RowsStage &st = sm.st[ring.s];
+            auto rowptr = [&](int r) { return r < safe_rp ? st.rp[r - ra] : rp[r]; };
+            const int p0 = rowptr(r0), p1 = rowptr(r1);
+            if (p1 - p0 <= kRowsBuf) {
+                const int oc = -(p0 & ~3), ov = -(p0 & ~1); // stage index = offset + global index
+                int q[RPT], e[RPT];
+                double s[RPT];
+#pragma unroll
+                for (int u = 0; u < RPT; ++u) {
+                    const int row = r0 + u * RSTRIDE + tid / LPR;
+                    q[u] = e[u] = 0;
+                    s[u] = 0.0;
+                    if (row < r1) {
+                        q[u] = rowptr(row) + gl;
+                        e[u] = rowptr(row + 1);
+                    }
+                }
+                bool more = true;
+                while (more) {
+                    int c[RPT][KU];
+#pragma unroll
+                    for (int u = 0; u < RPT; ++u)
+#pragma unroll
+                        for (int k = 0; k < KU; ++k) {
+                            const int g = q[u] + k * LPR;
+                            c[u][k] = 0;
+                            if (g < e[u]) c[u][k] = g < safe_ci ? st.ci[oc + g] : ci[g];
+                        }
+                    double xv[RPT][KU];
+#pragma unroll
+                    for (int u = 0; u < RPT; ++u)
+#pragma unroll
+                        for (int k = 0; k < KU; ++k) xv[u][k] = __ldg(x + c[u][k]);
+                    more = false;
+#pragma unroll
+                    for (int u = 0; u < RPT; ++u) {
+#pragma unroll
+                        for (int k = 0; k < KU; ++k) {
+                            const int g = q[u] + k * LPR;
+                            if (g < e[u]) s[u] = fma(g < safe_va ? st.va[ov + g] : va[g], xv[u][k], s[u]);
+                        }
+                        q[u] += KU * LPR;
+                        more |= q[u] < e[u];
+                    }
+                    more = __any_sync(0xffffffffu, more);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&sm.empty[ring.s]);
+#pragma unroll
+                for (int u = 0; u < RPT; ++u) {
+#pragma unroll
+                    for (int o = LPR / 2; o > 0; o >>= 1) s[u] += __shfl_xor_sync(0xffffffffu, s[u], o);
+                    const int row = r0 + u * RSTRIDE + tid / LPR;
+                    if (row < r1 && gl == 0) {
+                        const double val = (a.mode == MODE_RESIDUAL) ? a.b[row] - s[u] : s[u];
+                        a.w[row] = val;
+                        ss = fma(val, val, ss);
+                        am = fmax(am, fabs(val));
+                    }
+                }
+            } else {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&sm.empty[ring.s]);
+                for (int r = r0 + warp; r < r1; r += kRowsThreads / 32) { // oversized block: warp per row from global
+                    double t = 0.0;
+                    for (int p = rp[r] + lane; p < rp[r + 1]; p += 32) t = fma(va[p], x[ci[p]], t);
+                    t = warp_sum(t);
+                    if (lane == 0) {
+                        const double val = (a.mode == MODE_RESIDUAL) ? a.b[r] - t : t;
+                        a.w[r] = val;
+                        ss = fma(val, val, ss);
+                        am = fmax(am, fabs(val));
+                    }
+                }
+            }
+            ring.advance(kRowsStages);
+        }
     }
-    blk_row[b] = (int32_t)lo;
+    block_norm_partials(a, ss, am, &a.ctl->tickets[2]);
 }
 
-cudaError_t build_row_blocks(cudaStream_t s, int64_t n, int64_t nnz, const int32_t *d_row_ptr, int nnz_per_block,
-                             int32_t **d_blk_row_out, int *nblk_out)
+template <int RPT, int LPR> static void launch_rows(cudaStream_t s, const SpmvArgs &a)
 {
-    (void)nnz_per_block;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(spmv_rows_kernel<RPT, LPR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RowsSmem));
+        attr_set = true;
+    }
+    constexpr int RB = kRowsThreads * RPT / LPR;
+    const int64_t nblk = (a.A.n + RB - 1) / RB;
+    const int grid = (int)(nblk < 2 * kNumSMs ? nblk : 2 * kNumSMs); // persistent: two CTAs per SM
+    spmv_rows_kernel<RPT, LPR><<<grid, kRowsCta, sizeof(RowsSmem), s>>>(a);
+}
+
+// Row partition of the streaming kernel: block b = rows [R(b), R(b+1)) with R(b) the first row r with
+// row_ptr[r] >= b*T, so a block holds whole rows and about T nonzeros.  One descriptor per block:
+// {first row, end row, first nonzero, end nonzero}.
+__global__ void row_blocks_kernel(int64_t n, const int32_t *__restrict__ rp, int T, int nblk, int4 *desc)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nblk) return;
+    auto first_row = [&](int64_t target) { // first r in [0, n] with rp[r] >= target
+        int64_t lo = 0, hi = n;
+        while (lo < hi) {
+            const int64_t mid = (lo + hi) >> 1;
+            if (rp[mid] >= target) hi = mid;
+            else lo = mid + 1;
+        }
+        return (int)lo;
+    };
+    const int r0 = first_row((int64_t)b * T);
+    const int r1 = (b == nblk - 1) ? (int)n : first_row((int64_t)(b + 1) * T);
+    desc[b] = make_int4(r0, r1, rp[r0], rp[r1]);
+}
+
+cudaError_t build_row_blocks(cudaStream_t s, int64_t n, int64_t nnz, const int32_t *d_row_ptr, int4 **d_desc_out,
+                             int *nblk_out)
+{
     const int nblk = (int)((nnz + kStreamT - 1) / kStreamT) + 1;
-    int32_t *blk = nullptr;
-    cudaError_t e = cudaMalloc(&blk, (size_t)(nblk + 1) * sizeof(int32_t));
+    int4 *desc = nullptr;
+    cudaError_t e = cudaMalloc(&desc, (size_t)nblk * sizeof(int4));
     if (e != cudaSuccess) return e;
-    row_blocks_kernel<<<(nblk + 1 + 255) / 256, 256, 0, s>>>(n, d_row_ptr, kStreamT, nblk, blk);
-    *d_blk_row_out = blk;
+    row_blocks_kernel<<<(nblk + 255) / 256, 256, 0, s>>>(n, d_row_ptr, kStreamT, nblk, desc);
+    *d_desc_out = desc;
     *nblk_out = nblk;
     return cudaGetLastError();
 }
@@ -299,11 +574,12 @@ int launch_nrm2(cudaStream_t s, const Scratch &sc, int64_t n, const double *x, i
 
 template <int LANES> static void launch_vec(cudaStream_t s, const SpmvArgs &a)
 {
-    constexpr int RPB = 256 / LANES;
-    int64_t grid = (a.A.n + RPB - 1) / RPB;
+    constexpr int RPB = 256 / LANES, U = 4;
+    int64_t grid = (a.A.n + RPB * U - 1) / (RPB * U);
     const int64_t cap = (int64_t)kNumSMs * 8;
     if (grid > cap) grid = cap;
-    spmv_vec_kernel<LANES><<<(int)grid, 256, 0, s>>>(a);
+    if (grid < 1) grid = 1;
+    spmv_vec_kernel<LANES, U><<<(int)grid, 256, 0, s>>>(a);
 }
 
 int launch_spmv(cudaStream_t s, const Scratch &sc, const CsrView &A, const double *x, const double *b, double *w,
@@ -333,6 +609,13 @@ int launch_spmv(cudaStream_t s, const Scratch &sc, const CsrView &A, const doubl
         spmv_stream_kernel<<<grid, kStreamThreads, 0, s>>>(a);
         break;
     }
+    // row-major kernel: 128 + rows per thread, or 144 + lanes per row
+    case 129: launch_rows<1, 1>(s, a); break;
+    case 130: launch_rows<2, 1>(s, a); break;
+    case 132: launch_rows<4, 1>(s, a); break;
+    case 146: launch_rows<1, 2>(s, a); break;
+    case 148: launch_rows<1, 4>(s, a); break;
+    case 152: launch_rows<1, 8>(s, a); break;
     default: return 0;
     }
     return 1;

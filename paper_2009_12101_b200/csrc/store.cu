@@ -23,52 +23,63 @@ struct StoreArgs {
     int *h_flag;                 // mapped host word: mirrors ctl->stop_after (may be null)
 };
 
-// One thread: apply rotations 1..j-1 to the new column, form rotation j, rotate g, decide whether
-// the cycle goes on (recurrence residual; breakdown, Fig. 1 l.12; iteration bound).
+// The control CTA: apply rotations 1..j-1 to the new column, form rotation j, rotate g, decide
+// whether the cycle goes on (recurrence residual; breakdown, Fig. 1 l.12; iteration
+// bound).  The column and the rotations are staged in shared memory by all threads (one round trip
+// to global memory); the recurrence itself is inherently sequential and runs in one thread.
 __device__ void givens_step(const StoreArgs &a)
 {
+    __shared__ double s_h[kMaxRestart + 2], s_cs[kMaxRestart], s_sn[kMaxRestart];
     Ctl *ctl = a.ctl;
     const CycleState &cy = a.cyc;
-    const int j = a.step, m = ctl->m;
-    double *h = cy.h;
-    const double hn = ctl->hn;
-    h[j] = hn;
-    for (int c = 0; c < j - 1; ++c) {
-        const double t = cy.cs[c] * h[c] + cy.sn[c] * h[c + 1];
-        h[c + 1] = -cy.sn[c] * h[c] + cy.cs[c] * h[c + 1];
-        h[c] = t;
+    const int j = a.step, m = ctl->m, tid = threadIdx.x, nt = blockDim.x;
+    for (int c = tid; c < j; c += nt) s_h[c] = cy.h[c];
+    for (int c = tid; c < j - 1; c += nt) {
+        s_cs[c] = cy.cs[c];
+        s_sn[c] = cy.sn[c];
     }
-    const double rho = hypot(h[j - 1], h[j]);
-    double cj = 1.0, sj = 0.0;
-    if (rho != 0.0) {
-        cj = h[j - 1] / rho;
-        sj = h[j] / rho;
-    }
-    cy.cs[j - 1] = cj;
-    cy.sn[j - 1] = sj;
-    h[j - 1] = rho;
-    h[j] = 0.0;
-    double *Rcol = cy.R + (size_t)(j - 1) * (m + 1);
-    for (int c = 0; c < j; ++c) Rcol[c] = h[c];
-    const double gj = cy.g[j - 1];
-    cy.g[j] = -sj * gj;
-    cy.g[j - 1] = cj * gj;
-    const double rec = fabs(cy.g[j]);
-    const int iters = ctl->iters + 1;
-    ctl->iters = iters;
-    ctl->k = j;
-    ctl->rel_rec = rec / ctl->bnorm;
-    if (cy.hist && iters - 1 < ctl->hist_cap) cy.hist[iters - 1] = rec / ctl->bnorm;
-    if (!isfinite(rec)) ctl->nonfinite = 1;
-    const bool stop = (rec <= ctl->tol_abs) || ctl->breakdown || (iters >= ctl->max_iters) || ctl->nonfinite ||
-                      !isfinite(rec);
-    if (stop) {
-        ctl->stop_after = j; // later steps of this cycle see step > stop_after and return at once
-        if (a.h_flag) {
-            *reinterpret_cast<volatile int *>(a.h_flag) = j;
-            __threadfence_system();
+    __syncthreads();
+    if (tid == 0) {
+        const double hn = ctl->hn;
+        double hc = s_h[0]; // h_c after the rotations applied so far
+        for (int c = 0; c < j - 1; ++c) {
+            const double hnext = s_h[c + 1];
+            const double t = s_cs[c] * hc + s_sn[c] * hnext;
+            hc = -s_sn[c] * hc + s_cs[c] * hnext;
+            s_h[c] = t;
+        }
+        const double rho = hypot(hc, hn);
+        double cj = 1.0, sj = 0.0;
+        if (rho != 0.0) {
+            cj = hc / rho;
+            sj = hn / rho;
+        }
+        cy.cs[j - 1] = cj;
+        cy.sn[j - 1] = sj;
+        s_h[j - 1] = rho;
+        const double gj = cy.g[j - 1];
+        cy.g[j] = -sj * gj;
+        cy.g[j - 1] = cj * gj;
+        const double rec = fabs(sj * gj);
+        const int iters = ctl->iters + 1;
+        ctl->iters = iters;
+        ctl->k = j;
+        ctl->rel_rec = rec / ctl->bnorm;
+        if (cy.hist && iters - 1 < ctl->hist_cap) cy.hist[iters - 1] = rec / ctl->bnorm;
+        if (!isfinite(rec)) ctl->nonfinite = 1;
+        const bool stop = (rec <= ctl->tol_abs) || ctl->breakdown || (iters >= ctl->max_iters) || ctl->nonfinite ||
+                          !isfinite(rec);
+        if (stop) {
+            ctl->stop_after = j; // later steps of this cycle see step > stop_after and return at once
+            if (a.h_flag) {
+                *reinterpret_cast<volatile int *>(a.h_flag) = j;
+                __threadfence_system();
+            }
         }
     }
+    __syncthreads();
+    double *Rcol = cy.R + (size_t)(j - 1) * (m + 1);
+    for (int c = tid; c < j; c += nt) Rcol[c] = s_h[c];
 }
 
 template <int FMT, int THREADS> __global__ void __launch_bounds__(THREADS) store_kernel(const StoreArgs a)
@@ -77,7 +88,7 @@ template <int FMT, int THREADS> __global__ void __launch_bounds__(THREADS) store
     constexpr int VEC = F::VEC;
     if (a.mode != MODE_HOOK && a.step > a.ctl->stop_after) return;
     if (a.has_cyc && a.mode == MODE_ORTH1 && blockIdx.x == gridDim.x - 1) { // the control CTA
-        if (threadIdx.x == 0) givens_step(a);
+        givens_step(a);
         return;
     }
     const double hn = a.d_hn ? *a.d_hn : a.hn_host;

@@ -50,6 +50,7 @@ def main(argv=None) -> int:
     ap.add_argument("--spmv", default="")
     ap.add_argument("--json", default="")
     ap.add_argument("--interleave", type=int, default=0, help="orth_interleave option: 0 auto, 1 blocked, 2 interleaved")
+    ap.add_argument("--spmv-kernel", default="0", help="comma list of spmv_kernel options to time (0 = auto)")
     ap.add_argument("--seg-kb", type=int, default=0, help="orth_seg_kb option: 0 auto, 1, 2, 4")
     args = ap.parse_args(argv)
     ks = [int(x) for x in args.k.split(",") if x]
@@ -93,11 +94,13 @@ def main(argv=None) -> int:
         from workloads import make_config
 
         p = make_config(name)
-        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
         x = torch.randn(p.A.n, dtype=torch.float64, device=dev, generator=g)
         y = torch.empty_like(x)
-        med, best = _time(lambda: s.k_spmv(x, y, want_norm=False), args.reps, flush, torch)
-        rows.append((f"spmv[{name}]", "fp64", 0, med, best, model.spmv_bytes(p.A.n, p.A.nnz)))
+        for kern in [int(v) for v in args.spmv_kernel.split(",")]:
+            s.set_option("spmv_kernel", kern)
+            s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+            med, best = _time(lambda: s.k_spmv(x, y, want_norm=False), args.reps, flush, torch)
+            rows.append((f"spmv[{name},opt={kern}]", "fp64", 0, med, best, model.spmv_bytes(p.A.n, p.A.nnz)))
     print(f"# n={n} reps={args.reps} flush={args.flush}  GB/s = algorithmic bytes / median time")
     print(f"{'kernel':28s} {'fmt':6s} {'k':>4s} {'median_us':>10s} {'best_us':>10s} {'MB':>9s} {'GB/s':>8s}")
     out = []

@@ -234,7 +234,7 @@ def test_cgs_closed_form(solver, fmt):
 
 # ------------------------------------------------------------------------------------------ SpMV
 @pytest.mark.parametrize("name,kw", [("C1", {}), ("C2", {"grid": 30}), ("C4", {"n": 60000}), ("C5", {"grid": 20})])
-@pytest.mark.parametrize("kernel", [0, 2, 4, 8, 16, 32, 64])
+@pytest.mark.parametrize("kernel", [0, 2, 4, 8, 16, 32, 64, 129, 130, 132, 146, 148, 152])
 def test_spmv_matches_oracle(name, kw, kernel):
     from paper_2009_12101_b200 import Solver
 
