@@ -33,6 +33,7 @@ FORMATS = ("fp64", "fp32", "fp16", "int32", "int16")
 FORMAT_BYTES = {"fp64": 8, "fp32": 4, "fp16": 2, "int32": 4, "int16": 2}
 METRIC = "arnoldi_iters_per_sec"
 UNIT = "iters/s"
+PROFILE_EVERY = 4       # CUDA-event brackets around the kernels of every 4th Arnoldi step of the timed region
 REF_ITERS = 40          # Arnoldi steps per format in one step of the reference arm / cpu_baseline
 WORKLOADS = {"C2": {}, "C1": {}, "C5": {}, "C4": {}, "C2small": {"name": "C2", "grid": 32}}
 
@@ -207,7 +208,7 @@ def run_ours(args) -> int:
     host = {k: torch.as_tensor(v).pin_memory() for k, v in
             (("row_ptr", p.A.row_ptr), ("col_idx", p.A.col_idx), ("vals", p.A.vals), ("b", p.b), ("x0", p.x0))}
     host["x"] = torch.empty(n, dtype=torch.float64).pin_memory()
-    solver.set_option("profile", 1)
+    solver.set_option("profile", PROFILE_EVERY)
 
     # -- device-resident arm: W warm-up steps, K timed steps --
     for _ in range(args.warmup):

@@ -131,7 +131,9 @@ const char *cbgmres_last_error(cbgmres_handle_t h);
 /* Tuning / test knobs, by name.  "spmv_kernel": 0 = choose from the row-length statistics,
  * L in {2,4,8,16,32} = L lanes per row, 64 = nnz-balanced streaming kernel.  "poll": 1 (default)
  * = the host stops launching a cycle's remaining steps once the device reports it left the cycle.
- * "profile": 1 = time every kernel family with CUDA events (see cbgmres_profile_get), default 0.
+ * "profile": N > 0 = time the kernels of every N-th Arnoldi step of a cycle with CUDA events (see
+ * cbgmres_profile_get; 1 = every step), default 0.  "pdl": 1 (default) = launch the step kernels with
+ * programmatic stream serialisation (each parks in griddepcontrol.wait until its predecessor is done).
  * "orth_fuse": 1 (default) = fuse the first update with the second pass's multi-dot (one read of V).
  * "orth_seg_kb": 0 (default, chosen per launch), 1, 2 or 4 = KB per column segment of the
  * Gram-Schmidt passes' row tiles.  "orth_interleave": 0 (default: short segments only), 1 = one
@@ -142,7 +144,7 @@ int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value);
 /* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
 int64_t cbgmres_launch_count(cbgmres_handle_t h);
 
-/* Per-kernel timing (option "profile" = 1): cbgmres_solve brackets every launch of the families
+/* Per-kernel timing (option "profile" = N): cbgmres_solve brackets the launches (of every N-th step) of the families
  * below with CUDA events on its stream and accumulates, per family, the device time, the
  * ALGORITHMIC bytes of those launches (S1 12 nnz + 4(n+1) + 16 n;
  * S2 j n B + 8 n; S3 j n B + 16 n; S4 (16 + B) n; a fused S3+S2' launch counts j n B + 16 n)

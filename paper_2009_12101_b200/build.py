@@ -17,7 +17,7 @@ SOURCES = ["orth.cu", "store.cu", "spmv.cu", "small.cu", "solver.cu"]
 HEADERS = ["internal.cuh", "device_utils.cuh", os.path.join("..", "..", "include", "cbgmres.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-FLAGS = [*ARCH, "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
+FLAGS = [*ARCH, "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC", *os.environ.get("CBG_EXTRA_NVCC_FLAGS", "").split()]
 
 
 def _stale() -> bool:

@@ -17,6 +17,46 @@ __device__ __forceinline__ uint4 ldg_stream128(const void *p)
     return r;
 }
 
+// ---- widening to binary64 without the conversion pipe ---------------------------------------------
+// cvt.f64.f32 / cvt.f64.s32 issue at a quarter of the fp64 FMA rate; at 2 bytes per entry the basis
+// delivers ~13 entries per clock and SM, which that pipe cannot convert.  These build the binary64
+// bit pattern with integer ops and fix the exponent (or remove the magic offset) with ONE fp64
+// operation.  All are exact for every finite input, subnormals and zeros included
+// (define CBG_DECODE_CVT to get the plain conversions back).
+#ifdef CBG_DECODE_CVT
+__device__ __forceinline__ double f32_bits_to_double(unsigned f) { return (double)__uint_as_float(f); }
+__device__ __forceinline__ double i32_to_double(int q) { return (double)q; }
+__device__ __forceinline__ void half2_to_doubles(unsigned w, double &lo, double &hi)
+{
+    const __half2 h = *reinterpret_cast<const __half2 *>(&w);
+    const float2 f = __half22float2(h); // exact widening
+    lo = (double)f.x;
+    hi = (double)f.y;
+}
+#else
+// binary32 -> binary64: sign | exponent field | 23 fraction bits placed at the top of the binary64
+// fraction; the value is off by the bias difference 2^(1023-127), restored by an exact multiply
+// (a binary32 subnormal becomes a binary64 subnormal that the multiply normalises).
+__device__ __forceinline__ double f32_bits_to_double(unsigned f)
+{
+    const unsigned hi = (unsigned)((int)f >> 3) & 0x8FFFFFFFu;
+    return __hiloint2double((int)hi, (int)(f << 29)) * 0x1p896;
+}
+// int32 -> binary64: 2^52 + 2^31 + q is exact in the binade of 2^52; subtract the offset.
+__device__ __forceinline__ double i32_to_double(int q)
+{
+    return __hiloint2double(0x43300000, q ^ (int)0x80000000) - 4503601774854144.0;
+}
+// two binary16 -> binary64, same idea with the bias difference 2^(1023-15).
+__device__ __forceinline__ void half2_to_doubles(unsigned w, double &lo, double &hi)
+{
+    const unsigned h1 = (unsigned)((int)w >> 6) & 0x81FFFC00u;
+    const unsigned h0 = (unsigned)((int)(w << 16) >> 6) & 0x81FFFC00u;
+    lo = __hiloint2double((int)h0, 0) * 0x1p1008;
+    hi = __hiloint2double((int)h1, 0) * 0x1p1008;
+}
+#endif
+
 // ---- storage formats ----------------------------------------------------------
 // VEC = entries per 128-bit load.  decode() widens one 128-bit payload word to VEC fp64 values
 // WITHOUT the per-vector scale: the fixed-point scale sigma_c is folded into the coefficient
@@ -40,10 +80,10 @@ template <> struct Fmt<CBGMRES_FP32> {
     static constexpr bool SCALED = false;
     __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
     {
-        d[0] = (double)__uint_as_float(r.x);
-        d[1] = (double)__uint_as_float(r.y);
-        d[2] = (double)__uint_as_float(r.z);
-        d[3] = (double)__uint_as_float(r.w);
+        d[0] = f32_bits_to_double(r.x);
+        d[1] = f32_bits_to_double(r.y);
+        d[2] = f32_bits_to_double(r.z);
+        d[3] = f32_bits_to_double(r.w);
     }
     __device__ static __forceinline__ double decode_one(const void *col, int64_t i)
     {
@@ -51,13 +91,7 @@ template <> struct Fmt<CBGMRES_FP32> {
     }
 };
 
-__device__ __forceinline__ void half2_to_doubles(unsigned w, double &lo, double &hi)
-{
-    const __half2 h = *reinterpret_cast<const __half2 *>(&w);
-    const float2 f = __half22float2(h); // exact widening
-    lo = (double)f.x;
-    hi = (double)f.y;
-}
+
 
 template <> struct Fmt<CBGMRES_FP16> {
     static constexpr int VEC = 8, BYTES = 2;
@@ -80,10 +114,10 @@ template <> struct Fmt<CBGMRES_INT32> {
     static constexpr bool SCALED = true;
     __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
     {
-        d[0] = (double)(int)r.x;
-        d[1] = (double)(int)r.y;
-        d[2] = (double)(int)r.z;
-        d[3] = (double)(int)r.w;
+        d[0] = i32_to_double((int)r.x);
+        d[1] = i32_to_double((int)r.y);
+        d[2] = i32_to_double((int)r.z);
+        d[3] = i32_to_double((int)r.w);
     }
     __device__ static __forceinline__ double decode_one(const void *col, int64_t i)
     {
@@ -99,8 +133,8 @@ template <> struct Fmt<CBGMRES_INT16> {
         const unsigned w[4] = {r.x, r.y, r.z, r.w};
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-            d[2 * i] = (double)(int)(short)(w[i] & 0xFFFFu);
-            d[2 * i + 1] = (double)((int)w[i] >> 16);
+            d[2 * i] = i32_to_double((int)(w[i] << 16) >> 16);
+            d[2 * i + 1] = i32_to_double((int)w[i] >> 16);
         }
     }
     __device__ static __forceinline__ double decode_one(const void *col, int64_t i)
@@ -243,6 +277,33 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src, uint32
                      smem_u32(dst_smem)),
                  "l"(src), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
+}
+
+// ---- programmatic dependent launch ------------------------------------------------------------------
+// The kernels of an Arnoldi step form a chain on one stream, each 10-100 us long.  Launched with
+// the programmatic-stream-serialisation attribute, the next kernel's CTAs are scheduled while the
+// tail of the previous one (its last-block-done final stage) is still running, and park in
+// griddepcontrol.wait until that grid has completed and flushed; nothing produced by a predecessor
+// is read before the wait.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+extern int g_use_pdl; // solver.cu ("pdl" option)
+
+template <class... KArgs, class... Args>
+inline cudaError_t launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = g_use_pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
 // Position in a ring of shared-memory stages and the parity of its mbarriers.

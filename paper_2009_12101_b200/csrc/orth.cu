@@ -91,8 +91,9 @@ __device__ __forceinline__ void consumer_bar()
 //   [2048, 4096)   hpart[2][128] per-row-half dot partials of the CTA (epilogue)
 //   [4096, ...)    wbuf[2][R]  ring of w tiles
 //   then           red[8][R]   per-column-warp partial V h of the current tile (UPD kinds)
+//   then           w1buf[R]    the new w of the current tile for the second sweep (UPD kinds)
 //   then           stages[ns][8][SEG] ring of column chunks
-__host__ __device__ constexpr int orth_fixed_smem(int R, bool has_upd) { return 4096 + 16 * R + (has_upd ? 64 * R : 0); }
+__host__ __device__ constexpr int orth_fixed_smem(int R, bool has_upd) { return 4096 + 16 * R + (has_upd ? 72 * R : 0); }
 
 template <int FMT, int F> struct Tile {
     using Fm = Fmt<FMT>;
@@ -116,6 +117,19 @@ template <int FMT, int F> struct Tile {
         else return stage + lc * SEG + wi * 16;
     }
 };
+
+// Inner product of one decoded payload word with the matching rows of w: two independent chains of
+// VEC/2 FMAs (a single chain of 8 dependent fp64 FMAs per word starves the pipe at 4 warps per scheduler).
+template <int VEC> __device__ __forceinline__ double word_dot(const double (&d)[VEC], const double *w)
+{
+    double t0 = d[0] * w[0], t1 = d[1] * w[1];
+#pragma unroll
+    for (int v = 2; v < VEC; v += 2) {
+        t0 = fma(d[v], w[v], t0);
+        t1 = fma(d[v + 1], w[v + 1], t1);
+    }
+    return t0 + t1;
+}
 
 // Decode the F payload words of this lane in column `lc` of `stage` and hand VEC doubles per word to
 // `fn(f, d)`.  RAGGED: rows at or beyond `rows` are forced to zero (the payload there is stale
@@ -143,7 +157,7 @@ __device__ __forceinline__ void for_words(const unsigned char *stage, int lc, in
 struct ConsumerCtx {
     uint64_t *full, *empty, *wfull, *wempty;
     const double *hs_s;
-    double *wbuf, *red;
+    double *wbuf, *red, *w1buf;
     unsigned char *stages;
     int ns, k, nst; // ring size, columns of this launch, stages per row tile
     int lane, cw, half, ct; // lane, column of the chunk, row half, consumer thread index
@@ -167,29 +181,34 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
         for (int r = rows + c.ct; r < R; r += kConsumers) wt[r] = 0.0;
         consumer_bar();
     }
-    auto load_w = [&](double (&wreg)[GV]) {
+    auto load_w = [&](const double *src, double (&wreg)[GV]) {
 #pragma unroll
         for (int f = 0; f < F; ++f)
 #pragma unroll
             for (int v = 0; v < VEC; v += 2) {
-                const double2 t = *reinterpret_cast<const double2 *>(wt + (wi0 + f * 32) * VEC + v);
+                const double2 t = *reinterpret_cast<const double2 *>(src + (wi0 + f * 32) * VEC + v);
                 wreg[f * VEC + v] = t.x;
                 wreg[f * VEC + v + 1] = t.y;
             }
     };
     auto release_w = [&]() {
+        if (RAGGED) fence_proxy_async(); // this tile's slot was patched through the generic proxy; the next writer is the TMA
+        __threadfence_block();
         __syncwarp();
         if (c.lane == 0) mbar_arrive(&c.wempty[wslot]);
     };
+    // A slot may only be handed back once the shared-memory loads from it have COMPLETED, not merely
+    // been issued: the arithmetic that consumes them can be scheduled after the arrive, and the
+    // producer's next TMA write would overtake the loads.  The CTA-scope fence waits for them.
     auto release_stage = [&](int s) {
+        __threadfence_block();
         __syncwarp();
         if (c.lane == 0) mbar_arrive(&c.empty[s]);
     };
 
     if (KIND == PASS_DOT) {
         double wreg[GV];
-        load_w(wreg);
-        release_w();
+        load_w(wt, wreg);
 #pragma unroll
         for (int st = 0; st < kMaxChunks / T::CPS; ++st) {
             if (st < c.nst) {
@@ -200,9 +219,7 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
                     if (st * T::STAGE_COLS + lc < c.k) {
                         const unsigned char *stg = c.stages + (size_t)ring.s * T::STAGE;
                         for_words<FMT, F, RAGGED>(stg, lc, wi0, rows, [&](int f, const double(&d)[VEC]) {
-#pragma unroll
-                            for (int v = 0; v < VEC; ++v)
-                                acc[st * T::CPS + i] = fma(d[v], wreg[f * VEC + v], acc[st * T::CPS + i]);
+                            acc[st * T::CPS + i] += word_dot<VEC>(d, &wreg[f * VEC]);
                         });
                     }
                 }
@@ -210,6 +227,7 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
                 ring.advance(c.ns);
             }
         }
+        release_w(); // only now: the values have been used, so the loads from the slot have completed
         return;
     }
 
@@ -249,24 +267,21 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
 #pragma unroll
         for (int q = 0; q < kColWarps; ++q) tot += c.red[q * R + r];
         const double wn = wt[r] - tot;
-        if (!RAGGED || r < rows) {
+        const bool live = !RAGGED || r < rows;
+        if (live) {
             a.w[r0 + r] = wn;
             ss = fma(wn, wn, ss);
             am = fmax(am, fabs(wn));
-            if (HAS_DOT) wt[r] = wn;
         }
+        if (HAS_DOT) c.w1buf[r] = live ? wn : 0.0; // kept apart from the TMA-written slot: no proxy fence
     }
     consumer_bar();
-    if (KIND == PASS_UPD) {
-        release_w();
-        return;
-    }
+    release_w();
+    if (KIND == PASS_UPD) return;
 
     // ---- second sweep over the resident chunks: u_c += sum_rows dec(V)[r, c] * w_new[r] -----------------
     double wreg[GV];
-    load_w(wreg);
-    fence_proxy_async(); // the slot was written through the generic proxy; the next writer is the TMA
-    release_w();
+    load_w(c.w1buf, wreg);
     Ring r2 = tile_start;
 #pragma unroll
     for (int st = 0; st < kMaxChunks / T::CPS; ++st) {
@@ -277,9 +292,7 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
                 if (st * T::STAGE_COLS + lc < c.k) {
                     const unsigned char *stg = c.stages + (size_t)r2.s * T::STAGE;
                     for_words<FMT, F, RAGGED>(stg, lc, wi0, rows, [&](int f, const double(&d)[VEC]) {
-#pragma unroll
-                        for (int v = 0; v < VEC; ++v)
-                            acc[st * T::CPS + i] = fma(d[v], wreg[f * VEC + v], acc[st * T::CPS + i]);
+                        acc[st * T::CPS + i] += word_dot<VEC>(d, &wreg[f * VEC]);
                     });
                 }
             }
@@ -380,6 +393,8 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
     constexpr int R = T::R, B = T::B;
     constexpr bool HAS_UPD = KIND != PASS_DOT, HAS_DOT = KIND != PASS_UPD;
     Ctl *ctl = a.ctl;
+    pdl_wait();
+    pdl_launch_dependents();
     if (a.mode == MODE_ORTH1 || a.mode == MODE_ORTH2) {
         if (a.step > ctl->stop_after) return;
         if (a.mode == MODE_ORTH2 && !ctl->reorth_flag) return;
@@ -479,7 +494,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
             }
         }
     } else {
-        ConsumerCtx c{full, empty, wfull, wempty, hs_s, wbuf, red, stages, ns, k, nst, lane, warp & 7, warp >> 3, tid};
+        ConsumerCtx c{full, empty, wfull, wempty, hs_s, wbuf, red, red + kColWarps * R, stages, ns, k, nst, lane, warp & 7, warp >> 3, tid};
         Ring ring;
         for (int i = 0; i < ntiles; ++i) {
             const int t = dir ? ntiles - 1 - i : i;
@@ -637,7 +652,7 @@ template <int FMT, int F, int KIND> int launch_inst(cudaStream_t s, OrthArgs &a)
     int64_t grid = (a.n + 63) / 64;
     if (grid > kNumSMs) grid = kNumSMs;
     const size_t smem = (size_t)orth_fixed_smem(T::R, KIND != PASS_DOT) + (size_t)a.nstages * T::STAGE;
-    orth_kernel<FMT, F, KIND><<<(int)grid, kOrthThreads, smem, s>>>(a, *map);
+    launch_chain(orth_kernel<FMT, F, KIND>, dim3((unsigned)grid), dim3(kOrthThreads), smem, s, a, *map);
     return 1;
 }
 

@@ -10,6 +10,8 @@ namespace cbg {
 // Leaves hs_c = -sigma_c * y_c, the coefficients with which the update kernel forms x += V_k y.
 template <bool SCALED> __global__ void __launch_bounds__(32) backsolve_kernel(Ctl *ctl, CycleState cy)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     const int k = ctl->k;
     if (k <= 0) return;
     __shared__ double t[kMaxRestart + 1];
@@ -32,8 +34,8 @@ template <bool SCALED> __global__ void __launch_bounds__(32) backsolve_kernel(Ct
 
 int launch_backsolve(cudaStream_t s, const Scratch &sc, const CycleState &cyc, int format)
 {
-    if (format == CBGMRES_INT32 || format == CBGMRES_INT16) backsolve_kernel<true><<<1, 32, 0, s>>>(sc.ctl, cyc);
-    else backsolve_kernel<false><<<1, 32, 0, s>>>(sc.ctl, cyc);
+    if (format == CBGMRES_INT32 || format == CBGMRES_INT16) launch_chain(backsolve_kernel<true>, dim3(1), dim3(32), 0, s, sc.ctl, cyc);
+    else launch_chain(backsolve_kernel<false>, dim3(1), dim3(32), 0, s, sc.ctl, cyc);
     return 1;
 }
 

@@ -17,6 +17,10 @@
 
 using namespace cbg;
 
+namespace cbg {
+int g_use_pdl = 1; // programmatic dependent launch of the step kernels ("pdl" option)
+}
+
 struct ProfSlot {
     cudaEvent_t a = nullptr, b = nullptr;
     int family = 0, step = 0, pass = 0;
@@ -47,7 +51,8 @@ struct cbgmres_ctx {
     int64_t launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     // optional per-kernel timing ("profile" option): event pairs around the launches of one cycle
-    int opt_profile = 0;
+    int opt_profile = 0; // 0 = off, N = bracket the launches of every N-th Arnoldi step of a cycle
+    bool prof_on = false;
     std::vector<ProfSlot> prof_slots;
     int prof_used = 0;
     int *h_reorth_log = nullptr; // mapped pinned [kMaxRestart + 2]: reorth_flag per step of the cycle
@@ -147,7 +152,7 @@ int validate_params(cbgmres_ctx *h, const cbgmres_params *p)
 // stream synchronisation, when the device's control block (k, reorth_log) is back on the host.
 void prof_begin(cbgmres_ctx *h, int family, int step, int pass, double bytes)
 {
-    if (!h->opt_profile) return;
+    if (!h->prof_on) return;
     if (h->prof_used == (int)h->prof_slots.size()) {
         ProfSlot sl;
         if (cudaEventCreate(&sl.a) != cudaSuccess || cudaEventCreate(&sl.b) != cudaSuccess) return;
@@ -163,7 +168,7 @@ void prof_begin(cbgmres_ctx *h, int family, int step, int pass, double bytes)
 
 void prof_end(cbgmres_ctx *h)
 {
-    if (!h->opt_profile || h->prof_used >= (int)h->prof_slots.size()) return;
+    if (!h->prof_on || h->prof_used >= (int)h->prof_slots.size()) return;
     cudaEventRecord(h->prof_slots[h->prof_used].b, h->stream);
     h->prof_used += 1;
 }
@@ -335,8 +340,13 @@ int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value)
         h->opt_fuse = value != 0;
         return CBGMRES_OK;
     }
+    if (!strcmp(name, "pdl")) {
+        g_use_pdl = value != 0;
+        return CBGMRES_OK;
+    }
     if (!strcmp(name, "profile")) {
-        h->opt_profile = value != 0;
+        if (value < 0 || value > 1024) return fail(h, CBGMRES_E_INVALID, "profile must be 0..1024");
+        h->opt_profile = (int)value;
         return CBGMRES_OK;
     }
     return fail(h, CBGMRES_E_INVALID, "unknown option");
@@ -441,6 +451,7 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
         *flag = INT_MAX;
         h->prof_used = 0;
         const int restarts_before = h->h_ctl->restarts;
+        h->prof_on = h->opt_profile != 0;
         // l.1: r0 = b - A x, beta, the stopping test on the explicit residual; v1 = r0 / beta
         prof_begin(h, CBGMRES_PROF_RESIDUAL, 0, 0, bytes_spmv + 8.0 * dn + bytes_store);
         h->launches += launch_spmv(s, h->sc, h->A, d_x, d_b, w, MODE_RESIDUAL, 0, &cy, h->d_flag);
@@ -449,6 +460,7 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
         prof_end(h);
         for (int j = 1; j <= m; ++j) {
             if (h->opt_poll && *flag < j) break; // the device already left this cycle
+            h->prof_on = h->opt_profile && (j % h->opt_profile == 0);
             const double bytes_dot = (double)j * dn * dB + 8.0 * dn, bytes_upd = (double)j * dn * dB + 16.0 * dn;
             // l.3-4: w = A v, omega = ||w||
             prof_begin(h, CBGMRES_PROF_SPMV, j, 0, bytes_spmv);
@@ -492,6 +504,7 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
             prof_end(h);
         }
         // l.16-17: R y = g ; x += V_k y  (k read on the device)
+        h->prof_on = h->opt_profile != 0;
         prof_begin(h, CBGMRES_PROF_XUPDATE, 0, 0, 0.0);
         h->launches += launch_backsolve(s, h->sc, cy, fmt);
         h->launches += launch_update(s, h->sc, bv, n, m, &dctl->k, cy.hs, d_x, MODE_XUPDATE, 0, sk);

@@ -117,6 +117,8 @@ __device__ __forceinline__ void block_norm_partials(const SpmvArgs &a, double ss
 // then all gathers of x -- three rounds of independent loads instead of 3 U dependent ones.
 template <int LANES, int U> __global__ void __launch_bounds__(256) spmv_vec_kernel(const SpmvArgs a)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     if (a.mode == MODE_STEP && a.step > a.ctl->stop_after) return;
     constexpr int RPB = 256 / LANES;
     const int sub = threadIdx.x / LANES, sl = threadIdx.x % LANES;
@@ -213,6 +215,8 @@ __device__ __forceinline__ double ldg_stream_f64(const double *p, uint64_t pol)
 
 __global__ void __launch_bounds__(kStreamThreads) spmv_stream_kernel(const SpmvArgs a)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     if (a.mode == MODE_STEP && a.step > a.ctl->stop_after) return;
     __shared__ double prod[kStreamBuf];
     const int32_t *__restrict__ rp = a.A.row_ptr;
@@ -336,6 +340,8 @@ struct RowsSmem {
 
 template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_rows_kernel(const SpmvArgs a)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     if (a.mode == MODE_STEP && a.step > a.ctl->stop_after) return;
     constexpr int RB = kRowsThreads * RPT / LPR, KU = kRowsGathers / RPT, RSTRIDE = kRowsThreads / LPR;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -444,6 +450,7 @@ template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_
                     }
                     more = __any_sync(0xffffffffu, more);
                 }
+                __threadfence_block(); // the stage's loads must have completed, not merely been issued
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&sm.empty[ring.s]);
 #pragma unroll
@@ -489,7 +496,7 @@ template <int RPT, int LPR> static void launch_rows(cudaStream_t s, const SpmvAr
     constexpr int RB = kRowsThreads * RPT / LPR;
     const int64_t nblk = (a.A.n + RB - 1) / RB;
     const int grid = (int)(nblk < 2 * kNumSMs ? nblk : 2 * kNumSMs); // persistent: two CTAs per SM
-    spmv_rows_kernel<RPT, LPR><<<grid, kRowsCta, sizeof(RowsSmem), s>>>(a);
+    launch_chain(spmv_rows_kernel<RPT, LPR>, dim3(grid), dim3(kRowsCta), sizeof(RowsSmem), s, a);
 }
 
 // Row partition of the streaming kernel: block b = rows [R(b), R(b+1)) with R(b) the first row r with
@@ -579,7 +586,7 @@ template <int LANES> static void launch_vec(cudaStream_t s, const SpmvArgs &a)
     const int64_t cap = (int64_t)kNumSMs * 8;
     if (grid > cap) grid = cap;
     if (grid < 1) grid = 1;
-    spmv_vec_kernel<LANES, U><<<(int)grid, 256, 0, s>>>(a);
+    launch_chain(spmv_vec_kernel<LANES, U>, dim3((unsigned)grid), dim3(256), 0, s, a);
 }
 
 int launch_spmv(cudaStream_t s, const Scratch &sc, const CsrView &A, const double *x, const double *b, double *w,
@@ -606,7 +613,7 @@ int launch_spmv(cudaStream_t s, const Scratch &sc, const CsrView &A, const doubl
     case 64: {
         int grid = A.nblk < kNumSMs * 6 ? A.nblk : kNumSMs * 6;
         if (grid < 1) grid = 1;
-        spmv_stream_kernel<<<grid, kStreamThreads, 0, s>>>(a);
+        launch_chain(spmv_stream_kernel, dim3(grid), dim3(kStreamThreads), 0, s, a);
         break;
     }
     // row-major kernel: 128 + rows per thread, or 144 + lanes per row

@@ -86,6 +86,8 @@ template <int FMT, int THREADS> __global__ void __launch_bounds__(THREADS) store
 {
     using F = Fmt<FMT>;
     constexpr int VEC = F::VEC;
+    pdl_wait();
+    pdl_launch_dependents();
     if (a.mode != MODE_HOOK && a.step > a.ctl->stop_after) return;
     if (a.has_cyc && a.mode == MODE_ORTH1 && blockIdx.x == gridDim.x - 1) { // the control CTA
         givens_step(a);
@@ -166,7 +168,7 @@ template <int FMT> static int launch_store_t(cudaStream_t s, const StoreArgs &a)
     if (grid > cap) grid = cap;
     if (grid < 1) grid = 1;
     if (a.has_cyc && a.mode == MODE_ORTH1) grid += 1; // + the control CTA (Givens update)
-    store_kernel<FMT, THREADS><<<(int)grid, THREADS, 0, s>>>(a);
+    launch_chain(store_kernel<FMT, THREADS>, dim3((unsigned)grid), dim3(THREADS), 0, s, a);
     return 1;
 }
 

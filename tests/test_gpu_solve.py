@@ -207,3 +207,24 @@ def test_invalid_solve_arguments():
             assert e.value.code == 1
     finally:
         s.destroy()
+
+
+@pytest.mark.parametrize("fmt", ["fp64", "fp16", "int16"])
+def test_full_size_c2_solve_is_bitwise_repeatable(fmt):
+    """Every reduction has a fixed order, so two solves of the same system give the same bits -- on
+    the full-size C2 matrix, where each CTA of the Gram-Schmidt passes owns many row tiles."""
+    from paper_2009_12101_b200 import Solver
+
+    p = make_config("C2")
+    s = Solver(0)
+    try:
+        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+        runs = []
+        for _ in range(3):
+            x, r = s.solve(p.b, p.x0, p.restart, p.rel_tol, 150, fmt, history=True)
+            runs.append((x.cpu().numpy(), r.rec_history.copy()))
+        for x, hist in runs[1:]:
+            assert np.array_equal(hist, runs[0][1])
+            assert np.array_equal(x, runs[0][0])
+    finally:
+        s.destroy()
