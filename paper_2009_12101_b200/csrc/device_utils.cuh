@@ -306,6 +306,19 @@ inline cudaError_t launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block,
     return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
+// Hand a shared-memory slot back to the producer (arrive on its "empty" mbarrier) -- but only once
+// the values loaded from it have been USED by every lane: loads that have merely been issued can be
+// overtaken by the producer's next TMA write into the slot (seen as wrong inner products; a
+// CTA-scope MEMBAR.SC also closes the window but costs ~400 cycles per release).  `dep` must be
+// computed from results that consumed every load from the slot; the warp vote needs it from all 32
+// lanes and its result is an input of the arrive, so neither can be scheduled before the uses.
+__device__ __forceinline__ unsigned dep_bits(double x) { return (unsigned)__double2hiint(x); }
+__device__ __forceinline__ void mbar_arrive_after_use(uint64_t *bar, int lane, unsigned dep)
+{
+    const unsigned b = __ballot_sync(0xffffffffu, dep != 0x7ff1a5a5u);
+    if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0]; // after %1" ::"r"(smem_u32(bar)), "r"(b) : "memory");
+}
+
 // Position in a ring of shared-memory stages and the parity of its mbarriers.
 struct Ring {
     int s = 0;

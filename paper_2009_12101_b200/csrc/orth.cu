@@ -42,6 +42,7 @@ constexpr int kChunkCols = kColWarps;
 constexpr int kMaxChunks = 16;                          // chunks per launch (accumulators live in registers)
 constexpr int kMaxRangeCols = kMaxChunks * kChunkCols;  // 128 columns per launch
 constexpr int kMaxStages = 8;
+constexpr int kWSlots = 4;                              // ring of w tiles: how many row tiles the producer may run ahead
 constexpr int kStageBytes = 32 * 1024;                  // 8 columns x 4 KB, 16 x 2 KB or 32 x 1 KB
 constexpr int kOrthSmemBytes = 225 * 1024;              // dynamic shared memory of one CTA (one CTA per SM)
 
@@ -86,14 +87,14 @@ __device__ __forceinline__ void consumer_bar()
 }
 
 // ---- shared-memory map of one CTA -------------------------------------------------------------------
-//   [0, 1024)      mbarriers: full[32], empty[32], wfull[2], wempty[2]
+//   [0, 1024)      mbarriers: full[8], empty[8], wfull[4], wempty[4]
 //   [1024, 2048)   hs_s[128]   update coefficients of this launch's columns
 //   [2048, 4096)   hpart[2][128] per-row-half dot partials of the CTA (epilogue)
-//   [4096, ...)    wbuf[2][R]  ring of w tiles
+//   [4096, ...)    wbuf[4][R]  ring of w tiles
 //   then           red[8][R]   per-column-warp partial V h of the current tile (UPD kinds)
 //   then           w1buf[R]    the new w of the current tile for the second sweep (UPD kinds)
 //   then           stages[ns][8][SEG] ring of column chunks
-__host__ __device__ constexpr int orth_fixed_smem(int R, bool has_upd) { return 4096 + 16 * R + (has_upd ? 72 * R : 0); }
+__host__ __device__ constexpr int orth_fixed_smem(int R, bool has_upd) { return 4096 + kWSlots * 8 * R + (has_upd ? 72 * R : 0); }
 
 template <int FMT, int F> struct Tile {
     using Fm = Fmt<FMT>;
@@ -191,19 +192,18 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
                 wreg[f * VEC + v + 1] = t.y;
             }
     };
-    auto release_w = [&]() {
+    // Slots are handed back with mbar_arrive_after_use: `dep` carries a data dependency on everything
+    // that was loaded from the slot (device_utils.cuh).
+    auto release_w = [&](unsigned dep) {
         if (RAGGED) fence_proxy_async(); // this tile's slot was patched through the generic proxy; the next writer is the TMA
-        __threadfence_block();
-        __syncwarp();
-        if (c.lane == 0) mbar_arrive(&c.wempty[wslot]);
+        mbar_arrive_after_use(&c.wempty[wslot], c.lane, dep);
     };
-    // A slot may only be handed back once the shared-memory loads from it have COMPLETED, not merely
-    // been issued: the arithmetic that consumes them can be scheduled after the arrive, and the
-    // producer's next TMA write would overtake the loads.  The CTA-scope fence waits for them.
-    auto release_stage = [&](int s) {
-        __threadfence_block();
-        __syncwarp();
-        if (c.lane == 0) mbar_arrive(&c.empty[s]);
+    auto release_stage = [&](int s, unsigned dep) { mbar_arrive_after_use(&c.empty[s], c.lane, dep); };
+    auto dep_of = [&](const double(&wreg)[GV]) { // one value per 128-bit load of the w tile
+        unsigned dep = 0;
+#pragma unroll
+        for (int i = 0; i < GV; i += 2) dep ^= dep_bits(wreg[i]);
+        return dep;
     };
 
     if (KIND == PASS_DOT) {
@@ -223,11 +223,14 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
                         });
                     }
                 }
-                release_stage(ring.s);
+                unsigned dep = 0;
+#pragma unroll
+                for (int i = 0; i < T::CPS; ++i) dep ^= dep_bits(acc[st * T::CPS + i]);
+                release_stage(ring.s, dep);
                 ring.advance(c.ns);
             }
         }
-        release_w(); // only now: the values have been used, so the loads from the slot have completed
+        release_w(dep_of(wreg));
         return;
     }
 
@@ -251,7 +254,12 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
                 });
             }
         }
-        if (KIND == PASS_UPD) release_stage(ring.s);
+        if (KIND == PASS_UPD) {
+            unsigned dep = 0; // p[f * VEC] has consumed word f of every column of the stage
+#pragma unroll
+            for (int f = 0; f < F; ++f) dep ^= dep_bits(p[f * VEC]);
+            release_stage(ring.s, dep);
+        }
         ring.advance(c.ns);
     }
     double *redw = c.red + c.cw * R;
@@ -276,7 +284,7 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
         if (HAS_DOT) c.w1buf[r] = live ? wn : 0.0; // kept apart from the TMA-written slot: no proxy fence
     }
     consumer_bar();
-    release_w();
+    release_w(dep_bits(ss)); // the tile of w was consumed by the stores of the new w and by the norms
     if (KIND == PASS_UPD) return;
 
     // ---- second sweep over the resident chunks: u_c += sum_rows dec(V)[r, c] * w_new[r] -----------------
@@ -296,7 +304,10 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
                     });
                 }
             }
-            release_stage(r2.s);
+            unsigned dep = 0;
+#pragma unroll
+            for (int i = 0; i < T::CPS; ++i) dep ^= dep_bits(acc[st * T::CPS + i]);
+            release_stage(r2.s, dep);
             r2.advance(c.ns);
         }
     }
@@ -411,11 +422,11 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
     uint64_t *full = reinterpret_cast<uint64_t *>(smem);
     uint64_t *empty = full + kMaxStages;
     uint64_t *wfull = empty + kMaxStages;
-    uint64_t *wempty = wfull + 2;
+    uint64_t *wempty = wfull + kWSlots;
     double *hs_s = reinterpret_cast<double *>(smem + 1024);
     double *hpart = reinterpret_cast<double *>(smem + 2048);
     double *wbuf = reinterpret_cast<double *>(smem + 4096);
-    double *red = wbuf + 2 * R;
+    double *red = wbuf + kWSlots * R;
     unsigned char *stages = smem + orth_fixed_smem(R, HAS_UPD);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -424,7 +435,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], kConsumerWarps);
         }
-        for (int s = 0; s < 2; ++s) {
+        for (int s = 0; s < kWSlots; ++s) {
             mbar_init(&wfull[s], 1);
             mbar_init(&wempty[s], kConsumerWarps);
         }
@@ -469,9 +480,9 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
             const int64_t r0 = row_begin + (int64_t)t * tile_stride;
             const int rows = (int)min((int64_t)R, row_end - r0);
             const uint32_t w_bytes = (uint32_t)(rows * 8) & ~15u;
-            const int wslot = i & 1;
+            const int wslot = i % kWSlots;
             if (lane == 0) {
-                mbar_wait(&wempty[wslot], ((i >> 1) & 1) ^ 1u);
+                mbar_wait(&wempty[wslot], ((i / kWSlots) & 1) ^ 1u);
                 mbar_expect_tx(&wfull[wslot], w_bytes);
                 if (w_bytes) bulk_g2s(wbuf + wslot * R, a.w + r0, w_bytes, &wfull[wslot]);
             }
@@ -500,8 +511,8 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
             const int t = dir ? ntiles - 1 - i : i;
             const int64_t r0 = row_begin + (int64_t)t * tile_stride;
             const int rows = (int)min((int64_t)R, row_end - r0);
-            if (rows == R) consume_tile<FMT, F, KIND, false>(c, a, r0, rows, i & 1, (i >> 1) & 1, ring, acc, ss, am);
-            else consume_tile<FMT, F, KIND, true>(c, a, r0, rows, i & 1, (i >> 1) & 1, ring, acc, ss, am);
+            if (rows == R) consume_tile<FMT, F, KIND, false>(c, a, r0, rows, i % kWSlots, (i / kWSlots) & 1, ring, acc, ss, am);
+            else consume_tile<FMT, F, KIND, true>(c, a, r0, rows, i % kWSlots, (i / kWSlots) & 1, ring, acc, ss, am);
         }
         // ---- CTA partials ------------------------------------------------------------------------------
         if (HAS_DOT) {
