@@ -19,41 +19,57 @@ __device__ __forceinline__ uint4 ldg_stream128(const void *p)
 
 // ---- widening to binary64 without the conversion pipe ---------------------------------------------
 // cvt.f64.f32 / cvt.f64.s32 issue at a quarter of the fp64 FMA rate; at 2 bytes per entry the basis
-// delivers ~13 entries per clock and SM, which that pipe cannot convert.  These build the binary64
-// bit pattern with integer ops and fix the exponent (or remove the magic offset) with ONE fp64
-// operation.  All are exact for every finite input, subnormals and zeros included
-// (define CBG_DECODE_CVT to get the plain conversions back).
+// delivers ~11 entries per clock and SM, which that pipe cannot convert.  These build a binary64 bit
+// pattern with integer ops.  For the floating-point formats the pattern is the value times the bias
+// difference 2^-S (S = 896 for binary32, 1008 for binary16; a subnormal input becomes a binary64
+// subnormal, which the fp64 pipe takes at full speed); the passes multiply the OTHER operand of
+// every product (the tile of w, the coefficients h_c) by 2^(S/2) once and the result by 2^(S/2)
+// once, so no per-entry multiply is left.  Scaling by a power of two commutes with rounding (no
+// intermediate leaves the normal range: that would need abs(value) < 2^-518 or >= 2^520), so the
+// results are bit-identical to widening first.  Fixed point: 2^52 + offset + q is exact in the
+// binade of 2^52; one fp64 subtraction removes the offset.
+// (Define CBG_DECODE_CVT to get the plain conversions back.)
 #ifdef CBG_DECODE_CVT
-__device__ __forceinline__ double f32_bits_to_double(unsigned f) { return (double)__uint_as_float(f); }
+constexpr double kPreF32 = 1.0, kPreF16 = 1.0;
+__device__ __forceinline__ double f32_bits_to_raw(unsigned f) { return (double)__uint_as_float(f); }
 __device__ __forceinline__ double i32_to_double(int q) { return (double)q; }
-__device__ __forceinline__ void half2_to_doubles(unsigned w, double &lo, double &hi)
+// F2F.F64.F16 / I2F.F64.S16 take either half of a 32-bit register: one instruction per entry
+__device__ __forceinline__ void half2_to_raw(unsigned w, double &lo, double &hi)
 {
-    const __half2 h = *reinterpret_cast<const __half2 *>(&w);
-    const float2 f = __half22float2(h); // exact widening
-    lo = (double)f.x;
-    hi = (double)f.y;
+    asm("{.reg .b16 l, h; mov.b32 {l, h}, %2; cvt.f64.f16 %0, l; cvt.f64.f16 %1, h;}" : "=d"(lo), "=d"(hi) : "r"(w));
+}
+__device__ __forceinline__ void i16x2_to_doubles(unsigned w, double &lo, double &hi)
+{
+    asm("{.reg .b16 l, h; mov.b32 {l, h}, %2; cvt.rn.f64.s16 %0, l; cvt.rn.f64.s16 %1, h;}" : "=d"(lo), "=d"(hi) : "r"(w));
 }
 #else
-// binary32 -> binary64: sign | exponent field | 23 fraction bits placed at the top of the binary64
-// fraction; the value is off by the bias difference 2^(1023-127), restored by an exact multiply
-// (a binary32 subnormal becomes a binary64 subnormal that the multiply normalises).
-__device__ __forceinline__ double f32_bits_to_double(unsigned f)
+constexpr double kPreF32 = 0x1p448, kPreF16 = 0x1p504;
+// binary32 -> value * 2^-896: sign | exponent field | 23 fraction bits at the top of the binary64 fraction.
+__device__ __forceinline__ double f32_bits_to_raw(unsigned f)
 {
     const unsigned hi = (unsigned)((int)f >> 3) & 0x8FFFFFFFu;
-    return __hiloint2double((int)hi, (int)(f << 29)) * 0x1p896;
+    return __hiloint2double((int)hi, (int)(f << 29));
 }
-// int32 -> binary64: 2^52 + 2^31 + q is exact in the binade of 2^52; subtract the offset.
+// int32 -> binary64: 2^52 + 2^31 + q, minus the offset.
 __device__ __forceinline__ double i32_to_double(int q)
 {
     return __hiloint2double(0x43300000, q ^ (int)0x80000000) - 4503601774854144.0;
 }
-// two binary16 -> binary64, same idea with the bias difference 2^(1023-15).
-__device__ __forceinline__ void half2_to_doubles(unsigned w, double &lo, double &hi)
+// two binary16 -> values * 2^-1008.
+__device__ __forceinline__ void half2_to_raw(unsigned w, double &lo, double &hi)
 {
     const unsigned h1 = (unsigned)((int)w >> 6) & 0x81FFFC00u;
     const unsigned h0 = (unsigned)((int)(w << 16) >> 6) & 0x81FFFC00u;
-    lo = __hiloint2double((int)h0, 0) * 0x1p1008;
-    hi = __hiloint2double((int)h1, 0) * 0x1p1008;
+    lo = __hiloint2double((int)h0, 0);
+    hi = __hiloint2double((int)h1, 0);
+}
+// two int16 -> binary64: flip both sign bits at once (q + 32768 as an unsigned 16-bit field), then
+// 2^52 + 32768 + q minus the offset.
+__device__ __forceinline__ void i16x2_to_doubles(unsigned w, double &lo, double &hi)
+{
+    const unsigned u = w ^ 0x80008000u;
+    lo = __hiloint2double(0x43300000, (int)(u & 0xFFFFu)) - 4503599627403264.0;
+    hi = __hiloint2double(0x43300000, (int)(u >> 16)) - 4503599627403264.0;
 }
 #endif
 
@@ -67,6 +83,7 @@ template <int FMT> struct Fmt;
 template <> struct Fmt<CBGMRES_FP64> {
     static constexpr int VEC = 2, BYTES = 8;
     static constexpr bool SCALED = false;
+    static constexpr double PRE = 1.0; // decode() yields value / PRE^2 (see "widening" above)
     __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
     {
         d[0] = __hiloint2double((int)r.y, (int)r.x);
@@ -78,12 +95,13 @@ template <> struct Fmt<CBGMRES_FP64> {
 template <> struct Fmt<CBGMRES_FP32> {
     static constexpr int VEC = 4, BYTES = 4;
     static constexpr bool SCALED = false;
+    static constexpr double PRE = kPreF32;
     __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
     {
-        d[0] = f32_bits_to_double(r.x);
-        d[1] = f32_bits_to_double(r.y);
-        d[2] = f32_bits_to_double(r.z);
-        d[3] = f32_bits_to_double(r.w);
+        d[0] = f32_bits_to_raw(r.x);
+        d[1] = f32_bits_to_raw(r.y);
+        d[2] = f32_bits_to_raw(r.z);
+        d[3] = f32_bits_to_raw(r.w);
     }
     __device__ static __forceinline__ double decode_one(const void *col, int64_t i)
     {
@@ -96,12 +114,13 @@ template <> struct Fmt<CBGMRES_FP32> {
 template <> struct Fmt<CBGMRES_FP16> {
     static constexpr int VEC = 8, BYTES = 2;
     static constexpr bool SCALED = false;
+    static constexpr double PRE = kPreF16;
     __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
     {
-        half2_to_doubles(r.x, d[0], d[1]);
-        half2_to_doubles(r.y, d[2], d[3]);
-        half2_to_doubles(r.z, d[4], d[5]);
-        half2_to_doubles(r.w, d[6], d[7]);
+        half2_to_raw(r.x, d[0], d[1]);
+        half2_to_raw(r.y, d[2], d[3]);
+        half2_to_raw(r.z, d[4], d[5]);
+        half2_to_raw(r.w, d[6], d[7]);
     }
     __device__ static __forceinline__ double decode_one(const void *col, int64_t i)
     {
@@ -112,6 +131,7 @@ template <> struct Fmt<CBGMRES_FP16> {
 template <> struct Fmt<CBGMRES_INT32> {
     static constexpr int VEC = 4, BYTES = 4;
     static constexpr bool SCALED = true;
+    static constexpr double PRE = 1.0;
     __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
     {
         d[0] = i32_to_double((int)r.x);
@@ -128,14 +148,13 @@ template <> struct Fmt<CBGMRES_INT32> {
 template <> struct Fmt<CBGMRES_INT16> {
     static constexpr int VEC = 8, BYTES = 2;
     static constexpr bool SCALED = true;
+    static constexpr double PRE = 1.0;
     __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
     {
-        const unsigned w[4] = {r.x, r.y, r.z, r.w};
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            d[2 * i] = i32_to_double((int)(w[i] << 16) >> 16);
-            d[2 * i + 1] = i32_to_double((int)w[i] >> 16);
-        }
+        i16x2_to_doubles(r.x, d[0], d[1]);
+        i16x2_to_doubles(r.y, d[2], d[3]);
+        i16x2_to_doubles(r.z, d[4], d[5]);
+        i16x2_to_doubles(r.w, d[6], d[7]);
     }
     __device__ static __forceinline__ double decode_one(const void *col, int64_t i)
     {

@@ -34,6 +34,19 @@ namespace cbg {
 
 enum PassKind : int { PASS_DOT = 0, PASS_UPD = 1, PASS_UPD_DOT = 2 };
 
+#ifdef CBG_TRACE // development aid: per-CTA time stamps (ns) of the last orth launch
+__device__ unsigned long long g_trace[160][48];
+__device__ __forceinline__ unsigned long long gtime()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define TR(i) (g_trace[blockIdx.x][(i)] = gtime())
+#else
+#define TR(i) ((void)0)
+#endif
+
 constexpr int kColWarps = 8;                            // columns per chunk: one per warp of a row half
 constexpr int kConsumerWarps = 2 * kColWarps;           // two row halves
 constexpr int kConsumers = kConsumerWarps * 32;
@@ -132,28 +145,72 @@ template <int VEC> __device__ __forceinline__ double word_dot(const double (&d)[
     return t0 + t1;
 }
 
-// Decode the F payload words of this lane in column `lc` of `stage` and hand VEC doubles per word to
-// `fn(f, d)`.  RAGGED: rows at or beyond `rows` are forced to zero (the payload there is stale
-// shared memory or padding and may decode to NaN).
-template <int FMT, int F, bool RAGGED, class Fn>
-__device__ __forceinline__ void for_words(const unsigned char *stage, int lc, int wi0, int rows, Fn &&fn)
+// The payload words of this lane in NC consecutive chunks of a stage (its column `cw` of each chunk,
+// F words per column): ALL loads are issued first, then every word is widened and handed to
+// `fn(i, f, d)` (chunk, word, VEC values / PRE^2).  With the loads up front and no branch in between
+// the NC * F independent decode + FMA chains interleave; one word at a time left every warp with a
+// single chain and the SM (4 warps per scheduler) half idle.  RAGGED: rows at or beyond `rows` are
+// forced to zero (the payload there is stale shared memory or padding and may decode to NaN).
+template <int FMT, int F, int NC, bool RAGGED, class Fn>
+__device__ __forceinline__ void for_stage_words(const unsigned char *stage, int cw, int wi0, int rows, Fn &&fn)
 {
     using T = Tile<FMT, F>;
+    uint4 raw[NC][F];
 #pragma unroll
-    for (int f = 0; f < F; ++f) {
-        const int wi = wi0 + f * 32;
-        if (RAGGED && wi * T::VEC >= rows) continue;
-        const uint4 raw = *reinterpret_cast<const uint4 *>(T::word_ptr(stage, lc, wi));
-        double d[T::VEC];
-        T::Fm::decode(raw, d);
-        if (RAGGED) {
+    for (int i = 0; i < NC; ++i)
 #pragma unroll
-            for (int v = 0; v < T::VEC; ++v)
-                if (wi * T::VEC + v >= rows) d[v] = 0.0;
+        for (int f = 0; f < F; ++f) {
+            const int wi = wi0 + f * 32;
+            if (RAGGED && wi * T::VEC >= rows) raw[i][f] = make_uint4(0u, 0u, 0u, 0u);
+            else raw[i][f] = *reinterpret_cast<const uint4 *>(T::word_ptr(stage, i * kChunkCols + cw, wi));
         }
-        fn(f, d);
+#pragma unroll
+    for (int i = 0; i < NC; ++i)
+#pragma unroll
+        for (int f = 0; f < F; ++f) {
+            double d[T::VEC];
+            T::Fm::decode(raw[i][f], d);
+            if (RAGGED) {
+                const int wi = wi0 + f * 32;
+#pragma unroll
+                for (int v = 0; v < T::VEC; ++v)
+                    if (wi * T::VEC + v >= rows) d[v] = 0.0;
+            }
+            fn(i, f, d);
+        }
+}
+
+// Dispatch on the number of chunks of the stage in which this warp's column exists (nv = CPS for
+// every stage but the last of a row tile).
+template <int FMT, int F, bool RAGGED, class Fn>
+__device__ __forceinline__ void for_valid_chunks(int nv, const unsigned char *stage, int cw, int wi0, int rows, Fn &&fn)
+{
+    constexpr int CPS = Tile<FMT, F>::CPS;
+    if (nv >= CPS) {
+        for_stage_words<FMT, F, CPS, RAGGED>(stage, cw, wi0, rows, fn);
+    } else if constexpr (CPS >= 2) {
+        if (nv == 1) for_stage_words<FMT, F, 1, RAGGED>(stage, cw, wi0, rows, fn);
+        if constexpr (CPS == 4) {
+            if (nv == 2) for_stage_words<FMT, F, 2, RAGGED>(stage, cw, wi0, rows, fn);
+            if (nv == 3) for_stage_words<FMT, F, 3, RAGGED>(stage, cw, wi0, rows, fn);
+        }
     }
 }
+
+// Location of a row of a w tile in shared memory.  A lane owns 16-byte payload words, i.e. VEC
+// consecutive rows = VEC * 8 bytes of w: read linearly, the lanes of a warp are 32 or 64 bytes apart
+// and every 128-bit load is a 2- or 4-way bank conflict (measured: ~1 us per tile for the 16-bit
+// formats, all sixteen warps stalled -- the whole k-independent cost of a pass).  The tiles are
+// therefore stored with the TMA 32-byte / 64-byte swizzle (16-byte chunk index XOR address bits
+// 7.. ), which spreads the lanes of a quarter warp over all eight 16-byte bank groups.  fp64
+// (16 bytes of w per word) needs none.
+template <int VEC> __device__ __forceinline__ double *wswz(double *p)
+{
+    if constexpr (VEC == 2) return p;
+    const uintptr_t a = reinterpret_cast<uintptr_t>(p);
+    return reinterpret_cast<double *>(a ^ (((a >> 7) & (VEC == 8 ? 3u : 1u)) << 4));
+}
+template <int VEC> __device__ __forceinline__ const double *wswz(const double *p) { return wswz<VEC>(const_cast<double *>(p)); }
 
 struct ConsumerCtx {
     uint64_t *full, *empty, *wfull, *wempty;
@@ -172,25 +229,44 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
 {
     using T = Tile<FMT, F>;
     constexpr int VEC = T::VEC, GV = T::GV, R = T::R;
+    constexpr double PRE = T::Fm::PRE;
     constexpr bool HAS_UPD = KIND != PASS_DOT, HAS_DOT = KIND != PASS_UPD;
     const int wi0 = c.half * T::WORDS_HALF + c.lane; // this lane's first 16-byte word in a column segment
     double *wt = c.wbuf + wslot * R;
 
     mbar_wait(&c.wfull[wslot], wph);
-    if (RAGGED) { // rows beyond the tile's end read as zero; an odd last row is fetched by hand
-        if ((rows & 1) && c.ct == 0) wt[rows - 1] = a.w[r0 + rows - 1];
-        for (int r = rows + c.ct; r < R; r += kConsumers) wt[r] = 0.0;
+    if (RAGGED) {
+        if constexpr (VEC == 2) { // 1D copy: rows beyond the tile's end read as zero; an odd last row is fetched by hand
+            if ((rows & 1) && c.ct == 0) wt[rows - 1] = a.w[r0 + rows - 1];
+            for (int r = rows + c.ct; r < R; r += kConsumers) wt[r] = 0.0;
+        } else { // 2D box over complete groups of VEC rows (beyond them: zero fill); the last n % VEC rows by hand
+            const int64_t nfull = a.n / VEC * VEC;
+            if (r0 + rows == a.n && nfull < a.n)
+                for (int r = (int)(nfull - r0) + c.ct; r < rows; r += kConsumers) *wswz<VEC>(wt + r) = a.w[r0 + r];
+            if (nfull == 0) // n < VEC: the map's single group is in range although incomplete
+                for (int r = rows + c.ct; r < VEC; r += kConsumers) *wswz<VEC>(wt + r) = 0.0;
+        }
         consumer_bar();
     }
+    // rows of w owned by this lane, pre-multiplied by PRE (see "widening" in device_utils.cuh)
     auto load_w = [&](const double *src, double (&wreg)[GV]) {
 #pragma unroll
         for (int f = 0; f < F; ++f)
 #pragma unroll
             for (int v = 0; v < VEC; v += 2) {
-                const double2 t = *reinterpret_cast<const double2 *>(src + (wi0 + f * 32) * VEC + v);
-                wreg[f * VEC + v] = t.x;
-                wreg[f * VEC + v + 1] = t.y;
+                const double2 t = *reinterpret_cast<const double2 *>(wswz<VEC>(src + (wi0 + f * 32) * VEC + v));
+                wreg[f * VEC + v] = (PRE == 1.0) ? t.x : t.x * PRE;
+                wreg[f * VEC + v + 1] = (PRE == 1.0) ? t.y : t.y * PRE;
             }
+    };
+    // chunks of stage `st` in which this warp's column exists
+    auto valid_chunks = [&](int st) {
+        const int left = c.k - st * T::STAGE_COLS - c.cw; // > 0 iff the column exists in chunk 0
+#ifdef CBG_PROBE_NV // development probe: cap the work per stage (0 = consumers only wait and release)
+        return left <= 0 ? 0 : min(min(T::CPS, CBG_PROBE_NV), (left + kChunkCols - 1) / kChunkCols);
+#else
+        return left <= 0 ? 0 : min(T::CPS, (left + kChunkCols - 1) / kChunkCols);
+#endif
     };
     // Slots are handed back with mbar_arrive_after_use: `dep` carries a data dependency on everything
     // that was loaded from the slot (device_utils.cuh).
@@ -213,16 +289,10 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
         for (int st = 0; st < kMaxChunks / T::CPS; ++st) {
             if (st < c.nst) {
                 mbar_wait(&c.full[ring.s], ring.ph);
-#pragma unroll
-                for (int i = 0; i < T::CPS; ++i) {
-                    const int lc = i * kChunkCols + c.cw; // column within the stage
-                    if (st * T::STAGE_COLS + lc < c.k) {
-                        const unsigned char *stg = c.stages + (size_t)ring.s * T::STAGE;
-                        for_words<FMT, F, RAGGED>(stg, lc, wi0, rows, [&](int f, const double(&d)[VEC]) {
-                            acc[st * T::CPS + i] += word_dot<VEC>(d, &wreg[f * VEC]);
-                        });
-                    }
-                }
+                const unsigned char *stg = c.stages + (size_t)ring.s * T::STAGE;
+                for_valid_chunks<FMT, F, RAGGED>(valid_chunks(st), stg, c.cw, wi0, rows, [&](int i, int f, const double(&d)[VEC]) {
+                    acc[st * T::CPS + i] += word_dot<VEC>(d, &wreg[f * VEC]);
+                });
                 unsigned dep = 0;
 #pragma unroll
                 for (int i = 0; i < T::CPS; ++i) dep ^= dep_bits(acc[st * T::CPS + i]);
@@ -234,26 +304,21 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
         return;
     }
 
-    // ---- update: p = sum_c dec(V)[rows, c] * hs_c over this warp's columns -----------------------------
+    // ---- update: p = sum_c dec(V)[rows, c] * hs_c over this warp's columns (hs_s holds PRE * hs_c) ------
     const Ring tile_start = ring;
     double p[GV];
 #pragma unroll
     for (int i = 0; i < GV; ++i) p[i] = 0.0;
     for (int st = 0; st < c.nst; ++st) {
+        double coef[T::CPS]; // zero beyond k
+#pragma unroll
+        for (int i = 0; i < T::CPS; ++i) coef[i] = c.hs_s[st * T::STAGE_COLS + i * kChunkCols + c.cw];
         mbar_wait(&c.full[ring.s], ring.ph);
+        const unsigned char *stg = c.stages + (size_t)ring.s * T::STAGE;
+        for_valid_chunks<FMT, F, RAGGED>(valid_chunks(st), stg, c.cw, wi0, rows, [&](int i, int f, const double(&d)[VEC]) {
 #pragma unroll
-        for (int i = 0; i < T::CPS; ++i) {
-            const int lc = i * kChunkCols + c.cw;
-            const int col = st * T::STAGE_COLS + lc;
-            if (col < c.k) {
-                const double coef = c.hs_s[col];
-                const unsigned char *stg = c.stages + (size_t)ring.s * T::STAGE;
-                for_words<FMT, F, RAGGED>(stg, lc, wi0, rows, [&](int f, const double(&d)[VEC]) {
-#pragma unroll
-                    for (int v = 0; v < VEC; ++v) p[f * VEC + v] = fma(d[v], coef, p[f * VEC + v]);
-                });
-            }
-        }
+            for (int v = 0; v < VEC; ++v) p[f * VEC + v] = fma(d[v], coef[i], p[f * VEC + v]);
+        });
         if (KIND == PASS_UPD) {
             unsigned dep = 0; // p[f * VEC] has consumed word f of every column of the stage
 #pragma unroll
@@ -267,21 +332,22 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
     for (int f = 0; f < F; ++f)
 #pragma unroll
         for (int v = 0; v < VEC; v += 2)
-            *reinterpret_cast<double2 *>(redw + (wi0 + f * 32) * VEC + v) = make_double2(p[f * VEC + v], p[f * VEC + v + 1]);
+            *reinterpret_cast<double2 *>(wswz<VEC>(redw + (wi0 + f * 32) * VEC + v)) = make_double2(p[f * VEC + v], p[f * VEC + v + 1]);
     consumer_bar();
     // new w of the tile: the eight partial row vectors are added in a fixed order
     for (int r = c.ct; r < R; r += kConsumers) {
         double tot = 0.0;
 #pragma unroll
-        for (int q = 0; q < kColWarps; ++q) tot += c.red[q * R + r];
-        const double wn = wt[r] - tot;
+        for (int q = 0; q < kColWarps; ++q) tot += *wswz<VEC>(c.red + q * R + r); // stored like the w tiles: conflict-free both ways
+        const double wo = *wswz<VEC>(wt + r);
+        const double wn = (PRE == 1.0) ? wo - tot : fma(-tot, PRE, wo); // tot * PRE is exact: one rounding either way
         const bool live = !RAGGED || r < rows;
         if (live) {
             a.w[r0 + r] = wn;
             ss = fma(wn, wn, ss);
             am = fmax(am, fabs(wn));
         }
-        if (HAS_DOT) c.w1buf[r] = live ? wn : 0.0; // kept apart from the TMA-written slot: no proxy fence
+        if (HAS_DOT) *wswz<VEC>(c.w1buf + r) = live ? wn : 0.0; // kept apart from the TMA-written slot: no proxy fence
     }
     consumer_bar();
     release_w(dep_bits(ss)); // the tile of w was consumed by the stores of the new w and by the norms
@@ -294,16 +360,10 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
 #pragma unroll
     for (int st = 0; st < kMaxChunks / T::CPS; ++st) {
         if (st < c.nst) {
-#pragma unroll
-            for (int i = 0; i < T::CPS; ++i) {
-                const int lc = i * kChunkCols + c.cw;
-                if (st * T::STAGE_COLS + lc < c.k) {
-                    const unsigned char *stg = c.stages + (size_t)r2.s * T::STAGE;
-                    for_words<FMT, F, RAGGED>(stg, lc, wi0, rows, [&](int f, const double(&d)[VEC]) {
-                        acc[st * T::CPS + i] += word_dot<VEC>(d, &wreg[f * VEC]);
-                    });
-                }
-            }
+            const unsigned char *stg = c.stages + (size_t)r2.s * T::STAGE;
+            for_valid_chunks<FMT, F, RAGGED>(valid_chunks(st), stg, c.cw, wi0, rows, [&](int i, int f, const double(&d)[VEC]) {
+                acc[st * T::CPS + i] += word_dot<VEC>(d, &wreg[f * VEC]);
+            });
             unsigned dep = 0;
 #pragma unroll
             for (int i = 0; i < T::CPS; ++i) dep ^= dep_bits(acc[st * T::CPS + i]);
@@ -322,75 +382,98 @@ template <int KIND, bool SCALED> __device__ void orth_finalize(const OrthArgs &a
 {
     constexpr bool HAS_UPD = KIND != PASS_DOT, HAS_DOT = KIND != PASS_UPD;
     constexpr int NW = kOrthThreads / 32;
+    constexpr int UNR = 19; // partials in flight per thread: the loads are L2 round trips, issue them together
     Ctl *ctl = a.ctl;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nb = gridDim.x;
     __shared__ int s_apply;
+    __shared__ double s_nrm[2 * NW];
     if (tid == 0) s_apply = 1;
-    __syncthreads();
-    if (HAS_UPD && a.last_range && warp == 0) {
-        double t = 0.0, m = 0.0;
-        for (int b = lane; b < nb; b += 32) {
-            t += __ldcg(&a.npart[b]);
-            m = fmax(m, __ldcg(&a.npart[kMaxGrid + b]));
-        }
-        t = warp_sum(t);
-        m = warp_max(m);
-        if (lane == 0) {
-            const double hn = sqrt(t);
-            if (a.mode == MODE_HOOK) {
-                ctl->hook_nrm2 = hn;
-                ctl->hook_amax = m;
-            } else if (a.mode == MODE_ORTH1) {
-                // Fig. 1 l.6-7: h_{j+1,j} := ||w||_2 ; re-orthogonalise iff h_{j+1,j} < eta * omega
-                const int flag = (ctl->reorth_mode == CBGMRES_REORTH_ALWAYS) ||
-                                 (ctl->reorth_mode == CBGMRES_REORTH_COND && hn < ctl->eta * ctl->omega);
-                ctl->hn = hn;
-                ctl->amax = m;
-                ctl->breakdown = (hn == 0.0);
-                ctl->reorth_flag = flag;
-                ctl->reorth_log[a.step] = (unsigned char)flag;
-                if (!isfinite(hn)) ctl->nonfinite = 1;
-                s_apply = flag;
-            } else if (a.mode == MODE_ORTH2) {
-                // Fig. 1 l.10-12: new norm; breakdown if it again fell below eta * (norm before the pass)
-                const double omega1 = ctl->hn;
-                ctl->hn = hn;
-                ctl->amax = m;
-                ctl->reorth_count += 1;
-                ctl->breakdown = (hn == 0.0) || (hn < ctl->eta * omega1);
-                if (!isfinite(hn)) ctl->nonfinite = 1;
+
+    // ---- loads first: every thread's share of the CTA partials, all in flight at once ----------------
+    double nt = 0.0, nm = 0.0; // norms: one CTA per thread (grid <= kOrthThreads)
+    if (HAS_UPD && a.last_range && tid < nb) {
+        nt = __ldcg(&a.npart[tid]);
+        nm = __ldcg(&a.npart[kMaxGrid + tid]);
+    }
+    // dots: columns padded to kc = 32, 64 or 128; 512 / kc slices of CTAs, slice sl adds CTAs
+    // [sl * per, (sl + 1) * per) of its column in a fixed order
+    const int kc = k <= 32 ? 32 : (k <= 64 ? 64 : 128);
+    const int nsl = 512 / kc, col = tid & (kc - 1), sl = tid / kc;
+    const int per = (nb + nsl - 1) / nsl;
+    double *part = scratch; // [nsl][kMaxRangeCols]
+    if (HAS_DOT && tid < 512) {
+        double sum = 0.0;
+        if (col < k) {
+            const int b1 = min(nb, (sl + 1) * per);
+            for (int b = sl * per; b < b1; b += UNR) {
+                double v[UNR];
+#pragma unroll
+                for (int u = 0; u < UNR; ++u) v[u] = (b + u < b1) ? __ldcg(&a.partials[(size_t)(b + u) * kLdp + col]) : 0.0;
+#pragma unroll
+                for (int u = 0; u < UNR; ++u) sum += v[u];
             }
+        }
+        part[sl * kMaxRangeCols + col] = sum;
+    }
+    if (HAS_UPD && a.last_range) {
+        nt = warp_sum(nt);
+        nm = warp_max(nm);
+        if (lane == 0) {
+            s_nrm[warp] = nt;
+            s_nrm[NW + warp] = nm;
         }
     }
     __syncthreads();
-    if (HAS_DOT) {
-        double *part = scratch; // [NW][kMaxRangeCols]
-        for (int cg = 0; cg < k; cg += 32) {
-            const int col = cg + lane;
-            if (col < k) {
-                double sum = 0.0;
-                for (int b = warp; b < nb; b += NW) sum += __ldcg(&a.partials[(size_t)b * kLdp + col]);
-                part[warp * kMaxRangeCols + col] = sum;
-            }
-        }
-        __syncthreads();
-        const bool apply = s_apply != 0;
-        for (int col = tid; col < k; col += kOrthThreads) {
-            double tot = 0.0;
+    if (HAS_UPD && a.last_range && tid == 0) {
+        double t = 0.0, m = 0.0;
 #pragma unroll
-            for (int q = 0; q < NW; ++q) tot += part[q * kMaxRangeCols + col];
-            const double sigma = SCALED ? a.scales[col] : 1.0;
+        for (int i = 0; i < NW; ++i) {
+            t += s_nrm[i];
+            m = fmax(m, s_nrm[NW + i]);
+        }
+        const double hn = sqrt(t);
+        if (a.mode == MODE_HOOK) {
+            ctl->hook_nrm2 = hn;
+            ctl->hook_amax = m;
+        } else if (a.mode == MODE_ORTH1) {
+            // Fig. 1 l.6-7: h_{j+1,j} := ||w||_2 ; re-orthogonalise iff h_{j+1,j} < eta * omega
+            const int flag = (ctl->reorth_mode == CBGMRES_REORTH_ALWAYS) ||
+                             (ctl->reorth_mode == CBGMRES_REORTH_COND && hn < ctl->eta * ctl->omega);
+            ctl->hn = hn;
+            ctl->amax = m;
+            ctl->breakdown = (hn == 0.0);
+            ctl->reorth_flag = flag;
+            ctl->reorth_log[a.step] = (unsigned char)flag;
+            if (!isfinite(hn)) ctl->nonfinite = 1;
+            s_apply = flag;
+        } else if (a.mode == MODE_ORTH2) {
+            // Fig. 1 l.10-12: new norm; breakdown if it again fell below eta * (norm before the pass)
+            const double omega1 = ctl->hn;
+            ctl->hn = hn;
+            ctl->amax = m;
+            ctl->reorth_count += 1;
+            ctl->breakdown = (hn == 0.0) || (hn < ctl->eta * omega1);
+            if (!isfinite(hn)) ctl->nonfinite = 1;
+        }
+    }
+    if (HAS_UPD && HAS_DOT) __syncthreads(); // s_apply
+    if (HAS_DOT) {
+        const bool apply = s_apply != 0;
+        for (int c = tid; c < k; c += kOrthThreads) {
+            double tot = 0.0;
+            for (int q = 0; q < nsl; ++q) tot += part[q * kMaxRangeCols + c];
+            const double sigma = SCALED ? a.scales[c] : 1.0;
             const double h = tot * sigma; // h_c = sigma_c * sum_i q_ic w_i
             if (KIND == PASS_DOT) {
-                if (a.mode == MODE_ORTH2) a.h_out[col] += h; // Fig. 1 l.9: h_{1:j,j} += u
-                else a.h_out[col] = h;
-                if (a.hs_out) a.hs_out[col] = h * sigma;     // coefficient of the raw payload in the update
+                if (a.mode == MODE_ORTH2) a.h_out[c] += h; // Fig. 1 l.9: h_{1:j,j} += u
+                else a.h_out[c] = h;
+                if (a.hs_out) a.hs_out[c] = h * sigma;     // coefficient of the raw payload in the update
             } else if (a.mode == MODE_HOOK) {
-                a.h_out[col] = h;
-                if (a.hs_out) a.hs_out[col] = h * sigma;
+                a.h_out[c] = h;
+                if (a.hs_out) a.hs_out[c] = h * sigma;
             } else if (apply) { // fused pass inside the solver: u only counts if the second pass fires (l.7-9)
-                a.h_out[col] += h;
-                a.hs_out[col] = h * sigma;
+                a.h_out[c] += h;
+                a.hs_out[c] = h * sigma;
             }
         }
     }
@@ -398,21 +481,27 @@ template <int KIND, bool SCALED> __device__ void orth_finalize(const OrthArgs &a
 }
 
 template <int FMT, int F, int KIND>
-__global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a, const __grid_constant__ CUtensorMap tmap)
+__global__ void __launch_bounds__(kOrthThreads, 1)
+    orth_kernel(const OrthArgs a, const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap wmap)
 {
     using T = Tile<FMT, F>;
     constexpr int R = T::R, B = T::B;
     constexpr bool HAS_UPD = KIND != PASS_DOT, HAS_DOT = KIND != PASS_UPD;
     Ctl *ctl = a.ctl;
+    if (threadIdx.x == 0) TR(0);
     pdl_wait();
     pdl_launch_dependents();
+    if (threadIdx.x == 0) TR(1);
+    // the control words this CTA needs, fetched together (each is an L2 round trip)
+    const int stop_after = __ldcg(&ctl->stop_after), reorth_flag = __ldcg(&ctl->reorth_flag), ctl_dir = __ldcg(&ctl->dir);
+    const int dk = a.d_k ? __ldcg(a.d_k) : 0;
     if (a.mode == MODE_ORTH1 || a.mode == MODE_ORTH2) {
-        if (a.step > ctl->stop_after) return;
-        if (a.mode == MODE_ORTH2 && !ctl->reorth_flag) return;
+        if (a.step > stop_after) return;
+        if (a.mode == MODE_ORTH2 && !reorth_flag) return;
     }
     int k = a.k;
     if (a.d_k) { // cycle-end x update: the number of basis vectors is only known on the device
-        k = min(a.k, *a.d_k - a.c0);
+        k = min(a.k, dk - a.c0);
         if (k <= 0) return;
     }
     const int nst = (k + T::STAGE_COLS - 1) / T::STAGE_COLS; // stages per row tile
@@ -442,7 +531,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (HAS_UPD)
-        for (int c = tid; c < kMaxRangeCols; c += kOrthThreads) hs_s[c] = (c < k) ? a.hs[c] : 0.0;
+        for (int c = tid; c < kMaxRangeCols; c += kOrthThreads) hs_s[c] = (c < k) ? a.hs[c] * T::Fm::PRE : 0.0;
     __syncthreads();
 
     // Row tiles of this CTA.  Blocked: one contiguous row range per CTA (a multiple of 64 rows, so
@@ -465,7 +554,8 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
         ntiles = (int)((row_end - row_begin + R - 1) / R);
         tile_stride = R;
     }
-    const int dir = (a.mode == MODE_HOOK) ? 0 : ctl->dir; // consecutive passes walk in opposite directions
+    const int dir = (a.mode == MODE_HOOK) ? 0 : ctl_dir; // consecutive passes walk in opposite directions
+    if (threadIdx.x == 0) TR(2);
 
     double acc[kMaxChunks];
 #pragma unroll
@@ -479,12 +569,16 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
             const int t = dir ? ntiles - 1 - i : i;
             const int64_t r0 = row_begin + (int64_t)t * tile_stride;
             const int rows = (int)min((int64_t)R, row_end - r0);
-            const uint32_t w_bytes = (uint32_t)(rows * 8) & ~15u;
+            const uint32_t w_bytes = (T::VEC == 2) ? ((uint32_t)(rows * 8) & ~15u) : (uint32_t)(R * 8);
             const int wslot = i % kWSlots;
             if (lane == 0) {
                 mbar_wait(&wempty[wslot], ((i / kWSlots) & 1) ^ 1u);
                 mbar_expect_tx(&wfull[wslot], w_bytes);
-                if (w_bytes) bulk_g2s(wbuf + wslot * R, a.w + r0, w_bytes, &wfull[wslot]);
+                if constexpr (T::VEC == 2) { // linear tile, 1D bulk copy
+                    if (w_bytes) bulk_g2s(wbuf + wslot * R, a.w + r0, w_bytes, &wfull[wslot]);
+                } else { // swizzled tile: box [VEC x R / VEC] of w seen as [n / VEC][VEC]
+                    tma_box_g2s(wbuf + wslot * R, &wmap, 0, (int)(r0 / T::VEC), &wfull[wslot]);
+                }
             }
             const int x0 = (int)(r0 * B / 8); // first 8-byte word of the tile inside a column
             for (int st = 0; st < nst; ++st) {
@@ -496,6 +590,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
                     mbar_expect_tx(&full[ring.s], nboxes * T::BOX_BYTES);
                 }
                 __syncwarp();
+                if (lane == 0 && i == 0 && st == 0) TR(30);
                 if (lane < nboxes) {
                     unsigned char *dst = stages + (size_t)ring.s * T::STAGE + lane * T::BOX_BYTES;
                     if (F == 4) tma_box_g2s(dst, &tmap, x0 + lane * (T::BOX_INNER / 8), c_first, &full[ring.s]);
@@ -504,6 +599,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
                 ring.advance(ns);
             }
         }
+        if (lane == 0) TR(31);
     } else {
         ConsumerCtx c{full, empty, wfull, wempty, hs_s, wbuf, red, red + kColWarps * R, stages, ns, k, nst, lane, warp & 7, warp >> 3, tid};
         Ring ring;
@@ -513,13 +609,15 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
             const int rows = (int)min((int64_t)R, row_end - r0);
             if (rows == R) consume_tile<FMT, F, KIND, false>(c, a, r0, rows, i % kWSlots, (i / kWSlots) & 1, ring, acc, ss, am);
             else consume_tile<FMT, F, KIND, true>(c, a, r0, rows, i % kWSlots, (i / kWSlots) & 1, ring, acc, ss, am);
+            if (tid == 0 && i < 16) TR(3 + i);
         }
+        if (tid == 0) TR(20);
         // ---- CTA partials ------------------------------------------------------------------------------
         if (HAS_DOT) {
             const double tot = butterfly_rec<kMaxChunks, 16>(acc, lane);
             if (butterfly_owner<kMaxChunks>(lane)) {
                 const int col = butterfly_col<kMaxChunks>(lane) * kChunkCols + (warp & 7);
-                hpart[(warp >> 3) * kMaxRangeCols + col] = tot;
+                hpart[(warp >> 3) * kMaxRangeCols + col] = tot * T::Fm::PRE; // acc holds sums / PRE
             }
         }
         if (HAS_UPD) {
@@ -544,8 +642,11 @@ __global__ void __launch_bounds__(kOrthThreads, 1) orth_kernel(const OrthArgs a,
         a.npart[blockIdx.x] = t;
         a.npart[kMaxGrid + blockIdx.x] = m;
     }
+    if (threadIdx.x == 0) TR(21);
     if (!last_block_done(&ctl->tickets[0])) return;
+    if (threadIdx.x == 0) TR(22);
     orth_finalize<KIND, T::Fm::SCALED>(a, k, reinterpret_cast<double *>(smem + 4096));
+    if (threadIdx.x == 0) TR(23);
 }
 
 // ---- launchers ---------------------------------------------------------------------------------------
@@ -648,6 +749,47 @@ const CUtensorMap *basis_map(const void *V, int64_t ld, int64_t n, int bytes, in
     return &e.map;
 }
 
+// w as a 2D array [n / VEC groups][VEC doubles] with box [VEC x R / VEC] and the 32/64-byte swizzle
+// (see wswz).  Only complete groups are in range; rows beyond them read as zero.
+const CUtensorMap *w_map(const double *w, int64_t n, int vec, int R)
+{
+    struct Entry {
+        const double *w = nullptr;
+        int64_t n = 0;
+        int vec = 0, R = 0;
+        CUtensorMap map;
+    };
+    static thread_local Entry cache[16];
+    static thread_local int next = 0;
+    for (Entry &e : cache)
+        if (e.w == w && e.n == n && e.vec == vec && e.R == R) return &e.map;
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) {
+        g_orth_error = 999;
+        return nullptr;
+    }
+    Entry &e = cache[next];
+    next = (next + 1) % 16;
+    e.w = nullptr;
+    const cuuint64_t groups = (cuuint64_t)(n / vec);
+    const cuuint64_t dims[2] = {(cuuint64_t)vec, groups ? groups : 1};
+    const cuuint64_t strides[1] = {(cuuint64_t)vec * 8};
+    const cuuint32_t box[2] = {(cuuint32_t)vec, (cuuint32_t)(R / vec)};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult rc = fn(&e.map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, const_cast<double *>(w), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, vec == 8 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_32B,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (rc != CUDA_SUCCESS) {
+        g_orth_error = (int)rc;
+        return nullptr;
+    }
+    e.w = w;
+    e.n = n;
+    e.vec = vec;
+    e.R = R;
+    return &e.map;
+}
+
 template <int FMT, int F, int KIND> int launch_inst(cudaStream_t s, OrthArgs &a)
 {
     using T = Tile<FMT, F>;
@@ -659,11 +801,13 @@ template <int FMT, int F, int KIND> int launch_inst(cudaStream_t s, OrthArgs &a)
     }
     const CUtensorMap *map = basis_map(a.V, a.ld, a.n, T::B, a.k, T::BOX_INNER);
     if (!map) return 0;
+    const CUtensorMap *wm = (T::VEC == 2) ? map : w_map(a.w, a.n, T::VEC, T::R); // fp64: linear w tiles, map unused
+    if (!wm) return 0;
     a.nstages = stages_for(FMT, F, KIND != PASS_DOT);
     int64_t grid = (a.n + 63) / 64;
     if (grid > kNumSMs) grid = kNumSMs;
     const size_t smem = (size_t)orth_fixed_smem(T::R, KIND != PASS_DOT) + (size_t)a.nstages * T::STAGE;
-    launch_chain(orth_kernel<FMT, F, KIND>, dim3((unsigned)grid), dim3(kOrthThreads), smem, s, a, *map);
+    launch_chain(orth_kernel<FMT, F, KIND>, dim3((unsigned)grid), dim3(kOrthThreads), smem, s, a, *map, *wm);
     return 1;
 }
 
@@ -711,6 +855,17 @@ OrthArgs base_args(const Scratch &sc, const BasisView &b, int64_t n, int mode, i
 } // namespace
 
 void set_orth_interleave(int v) { g_interleave_opt = v; }
+#ifdef CBG_TRACE
+extern "C" int cbgmres_debug_trace(unsigned long long *host_out)
+{
+    return (int)cudaMemcpyFromSymbol(host_out, g_trace, sizeof(g_trace));
+}
+extern "C" int cbgmres_debug_trace_clear()
+{
+    static unsigned long long z[160][48];
+    return (int)cudaMemcpyToSymbol(g_trace, z, sizeof(z));
+}
+#endif
 int take_orth_error()
 {
     const int e = g_orth_error;

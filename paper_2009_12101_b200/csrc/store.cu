@@ -40,12 +40,18 @@ __device__ void givens_step(const StoreArgs &a)
     }
     __syncthreads();
     if (tid == 0) {
-        const double hn = ctl->hn;
+        // scalars of the control block, fetched together (L2 round trips) before the recurrence
+        const double hn = __ldcg(&ctl->hn), bnorm = __ldcg(&ctl->bnorm), tol_abs = __ldcg(&ctl->tol_abs);
+        const double gj = __ldcg(&cy.g[j - 1]);
+        const int iters0 = __ldcg(&ctl->iters), max_iters = __ldcg(&ctl->max_iters), hist_cap = __ldcg(&ctl->hist_cap);
+        const int bd = __ldcg(&ctl->breakdown), nonfin = __ldcg(&ctl->nonfinite);
         double hc = s_h[0]; // h_c after the rotations applied so far
         for (int c = 0; c < j - 1; ++c) {
+            // one FMA per rotation on the critical path: the products with h_{c+1} do not depend on hc
             const double hnext = s_h[c + 1];
-            const double t = s_cs[c] * hc + s_sn[c] * hnext;
-            hc = -s_sn[c] * hc + s_cs[c] * hnext;
+            const double a1 = s_sn[c] * hnext, a2 = s_cs[c] * hnext;
+            const double t = fma(s_cs[c], hc, a1);
+            hc = fma(-s_sn[c], hc, a2);
             s_h[c] = t;
         }
         const double rho = hypot(hc, hn);
@@ -57,18 +63,16 @@ __device__ void givens_step(const StoreArgs &a)
         cy.cs[j - 1] = cj;
         cy.sn[j - 1] = sj;
         s_h[j - 1] = rho;
-        const double gj = cy.g[j - 1];
         cy.g[j] = -sj * gj;
         cy.g[j - 1] = cj * gj;
         const double rec = fabs(sj * gj);
-        const int iters = ctl->iters + 1;
+        const int iters = iters0 + 1;
         ctl->iters = iters;
         ctl->k = j;
-        ctl->rel_rec = rec / ctl->bnorm;
-        if (cy.hist && iters - 1 < ctl->hist_cap) cy.hist[iters - 1] = rec / ctl->bnorm;
+        ctl->rel_rec = rec / bnorm;
+        if (cy.hist && iters - 1 < hist_cap) cy.hist[iters - 1] = rec / bnorm;
         if (!isfinite(rec)) ctl->nonfinite = 1;
-        const bool stop = (rec <= ctl->tol_abs) || ctl->breakdown || (iters >= ctl->max_iters) || ctl->nonfinite ||
-                          !isfinite(rec);
+        const bool stop = (rec <= tol_abs) || bd || (iters >= max_iters) || nonfin || !isfinite(rec);
         if (stop) {
             ctl->stop_after = j; // later steps of this cycle see step > stop_after and return at once
             if (a.h_flag) {
@@ -88,13 +92,18 @@ template <int FMT, int THREADS> __global__ void __launch_bounds__(THREADS) store
     constexpr int VEC = F::VEC;
     pdl_wait();
     pdl_launch_dependents();
-    if (a.mode != MODE_HOOK && a.step > a.ctl->stop_after) return;
-    if (a.has_cyc && a.mode == MODE_ORTH1 && blockIdx.x == gridDim.x - 1) { // the control CTA
+    // control words fetched together (each is an L2 round trip)
+    const int stop_after = (a.mode != MODE_HOOK) ? __ldcg(&a.ctl->stop_after) : 0;
+    const double hn_dev = a.d_hn ? __ldcg(a.d_hn) : 0.0, amax_dev = a.d_amax ? __ldcg(a.d_amax) : 0.0;
+    if (a.mode != MODE_HOOK && a.step > stop_after) return;
+    const bool has_ctl_cta = a.has_cyc && a.mode == MODE_ORTH1;
+    if (has_ctl_cta && blockIdx.x == 0) { // the control CTA: first to be scheduled, its serial chain overlaps the streaming
         givens_step(a);
         return;
     }
-    const double hn = a.d_hn ? *a.d_hn : a.hn_host;
-    const double amax_w = a.d_amax ? *a.d_amax : a.amax_host;
+    const int bid = has_ctl_cta ? blockIdx.x - 1 : blockIdx.x;
+    const double hn = a.d_hn ? hn_dev : a.hn_host;
+    const double amax_w = a.d_amax ? amax_dev : a.amax_host;
     if (!(hn > 0.0)) return; // Fig. 1 l.12: h_{j+1,j} = 0 -> no new vector
     double s = 0.0, sigma = 1.0;
     if (F::SCALED) {
@@ -109,11 +118,11 @@ template <int FMT, int THREADS> __global__ void __launch_bounds__(THREADS) store
             sigma = 0.0;
         }
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) *a.scale_out = sigma;
+    if (bid == 0 && threadIdx.x == 0) *a.scale_out = sigma;
 
-    const int nblk = a.has_cyc && a.mode == MODE_ORTH1 ? gridDim.x - 1 : gridDim.x;
+    const int nblk = has_ctl_cta ? gridDim.x - 1 : gridDim.x;
     const int64_t ngroups = (a.n + VEC - 1) / VEC;
-    for (int64_t g = (int64_t)blockIdx.x * THREADS + threadIdx.x; g < ngroups; g += (int64_t)nblk * THREADS) {
+    for (int64_t g = (int64_t)bid * THREADS + threadIdx.x; g < ngroups; g += (int64_t)nblk * THREADS) {
         const int64_t row = g * VEC;
         if (row + VEC <= a.n) {
             double v[VEC];
