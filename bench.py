@@ -180,6 +180,22 @@ def _solve_all_formats(solver, p, dev, host=None):
     return out
 
 
+def aggregate_over_ranks(world: int, device, ms: float, e_ms: float, iters: int, e_iters: int, launches: int):
+    """Whole-job figures of N independent replicas ("replicas only"): the timed
+    regions are bracketed by barriers, so the job takes the MAX of the ranks' times; iterations and
+    launches are SUMMED.  No data-path collective exists; this is the only cross-rank exchange."""
+    if world <= 1:
+        return ms, e_ms, iters, e_iters, launches
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([ms, e_ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([iters, e_iters, launches], dtype=torch.float64, device=device)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t[0]), float(t[1]), int(c[0]), int(c[1]), int(c[2])
+
+
 def run_ours(args) -> int:
     import torch
     import torch.distributed as dist
@@ -241,15 +257,7 @@ def run_ours(args) -> int:
     h2d = nf * (4 * (n + 1) + 12 * nnz + 16 * n)
     d2h = nf * 8 * n
 
-    if world > 1:
-        t = torch.tensor([ms, e_s * 1e3], dtype=torch.float64, device=solver.device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        c = torch.tensor([iters, e_iters, launches], dtype=torch.float64, device=solver.device)
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        ms, e_ms = float(t[0]), float(t[1])
-        iters, e_iters, launches = int(c[0]), int(c[1]), int(c[2])
-    else:
-        e_ms = e_s * 1e3
+    ms, e_ms, iters, e_iters, launches = aggregate_over_ranks(world, solver.device, ms, e_s * 1e3, iters, e_iters, launches)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

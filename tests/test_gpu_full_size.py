@@ -1,0 +1,161 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configurations bench.py and the C3
+microbench time: outputs the oracle can compute one by one are compared on samples (columns of
+the multi-dot, rows of the update, every row of the SpMV -- the oracle's SpMV is fast enough), the
+rest through properties that hold at any size (norms of the GPU's own output, true residuals,
+residual histories over a bounded prefix of the solve)."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_config
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-12
+N_C3 = 4_194_304  # BASELINE.json configs[2]
+
+
+def _dev(a):
+    import torch
+
+    return torch.as_tensor(np.ascontiguousarray(a), device="cuda")
+
+
+@pytest.fixture(scope="module")
+def solver():
+    from paper_2009_12101_b200 import Solver
+
+    s = Solver(0)
+    yield s
+    s.destroy()
+
+
+@pytest.fixture(scope="module")
+def c3_vectors():
+    """k = 100 vectors of n = 4,194,304 entries of typical size n^-1/2 (the value distribution of the
+    decode path), scaled to unit 2-norm; w standard normal.  No QR at this
+    size (minutes on the host): orthogonality plays no role in per-kernel parity."""
+    rng = np.random.default_rng(2)
+    k = 100
+    V = rng.standard_normal((k, N_C3))
+    V /= np.linalg.norm(V, axis=1, keepdims=True)
+    w = rng.standard_normal(N_C3)
+    h = rng.standard_normal(k)
+    return V, w, h
+
+
+@pytest.mark.parametrize("fmt", ["fp32", "int16"])
+def test_c3_size_passes_sampled(solver, c3_vectors, fmt):
+    import torch
+    from paper_2009_12101_b200 import payload_dtype
+
+    V, w, h = c3_vectors
+    k, n = V.shape
+    P, sig = oracle.enc_basis(fmt, V)
+    dP = torch.as_tensor(P, device="cuda").view(payload_dtype(fmt))
+    dsig, dw = _dev(sig), _dev(w)
+    wn = np.linalg.norm(w)
+
+    # S2: sampled columns against the oracle's extended-precision dot
+    cols = [0, 1, 37, 63, 64, 99]
+    hg = solver.k_multidot(fmt, dP, dsig, dw, n=n, k=k).cpu().numpy()
+    assert np.all(np.isfinite(hg))
+    for c in cols:
+        ref = oracle.ref_multidot(fmt, P[c:c + 1], sig[c:c + 1], w, k=1)[0]
+        vn = np.linalg.norm(oracle.dec(fmt, P[c], sig[c]))
+        assert abs(hg[c] - ref) <= TOL * vn * wn
+
+    # S3 (+ S2' fused): sampled rows -- first and last tiles, tile borders, random interior rows
+    rng = np.random.default_rng(7)
+    rows = np.unique(np.concatenate([np.arange(0, 2048), np.arange(n - 2048, n),
+                                     rng.integers(0, n, 4096), np.arange(1 << 20, (1 << 20) + 64)]))
+    w_ref_rows, _, _ = oracle.ref_update(fmt, np.ascontiguousarray(P[:, rows]), sig, h, w[rows])
+    row_tol = TOL * (np.abs(w[rows]) + np.linalg.norm(h))  # |dw_i| <= tol (|w_i| + ||V^_{i,:}|| ||h||), ||V^_{i,:}|| << 1
+
+    d1 = dw.clone()
+    out = solver.k_update(fmt, dP, dsig, _dev(h), d1, n=n)
+    torch.cuda.synchronize()
+    w1 = d1.cpu().numpy()
+    nrm2, amax = out.cpu().numpy()
+    assert np.all(np.abs(w1[rows] - w_ref_rows) <= row_tol)
+    assert abs(nrm2 - np.linalg.norm(w1)) <= 1e-13 * np.linalg.norm(w1)  # the norm of the kernel's own output
+    assert amax == np.abs(w1).max()
+
+    d2 = dw.clone()
+    u, out2 = solver.k_update_multidot(fmt, dP, dsig, _dev(h), d2, n=n)
+    torch.cuda.synchronize()
+    w2 = d2.cpu().numpy()
+    assert np.all(np.abs(w2[rows] - w_ref_rows) <= row_tol)
+    nrm2f, amaxf = out2.cpu().numpy()
+    assert abs(nrm2f - np.linalg.norm(w2)) <= 1e-13 * np.linalg.norm(w2)
+    assert amaxf == np.abs(w2).max()
+    ug = u.cpu().numpy()
+    for c in cols:  # u = dec(V)^T w_new, on the GPU's own w_new (exactly representable input for the oracle)
+        ref = oracle.ref_multidot(fmt, P[c:c + 1], sig[c:c + 1], w2, k=1)[0]
+        vn = np.linalg.norm(oracle.dec(fmt, P[c], sig[c]))
+        assert abs(ug[c] - ref) <= TOL * vn * np.linalg.norm(w2)
+
+
+@pytest.mark.parametrize("name", ["C2", "C4", "C5"])
+def test_full_size_spmv_every_row(name):
+    """S1 on the full-size matrices with the kernel set_matrix selects (the one bench.py times)."""
+    from paper_2009_12101_b200 import Solver
+
+    p = make_config(name)
+    s = Solver(0)
+    try:
+        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+        x = np.random.default_rng(600).standard_normal(p.A.n)
+        y_ref, rowabs = oracle.ref_spmv(p.A, x)
+        w, nrm = s.k_spmv(_dev(x))
+        y = w.cpu().numpy()
+        assert np.all(np.abs(y - y_ref) <= TOL * np.maximum(rowabs, 1e-300))
+        assert abs(nrm.item() - np.linalg.norm(y_ref)) <= TOL * np.linalg.norm(y_ref)
+    finally:
+        s.destroy()
+
+
+@pytest.fixture(scope="module")
+def c2_full():
+    from paper_2009_12101_b200 import Solver
+
+    p = make_config("C2")
+    s = Solver(0)
+    s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+    yield p, s
+    s.destroy()
+
+
+@pytest.mark.parametrize("fmt", oracle.FORMATS)
+def test_full_size_c2_solve_properties(c2_full, fmt):
+    """The solve bench.py times.  Properties: converged, the explicit residual of the returned x
+    (recomputed with the oracle's SpMV) is below tolerance and equals the reported one."""
+    p, s = c2_full
+    x, r = s.solve(p.b, p.x0, p.restart, p.rel_tol, p.max_iters, fmt)
+    xh = x.cpu().numpy()
+    true = np.linalg.norm(p.b - oracle.spmv(p.A, xh)) / np.linalg.norm(p.b)
+    assert r.converged
+    assert true <= p.rel_tol * (1 + 1e-9)
+    assert r.rel_res_true == pytest.approx(true, rel=1e-6)
+    assert r.iters <= p.max_iters and r.restarts >= r.iters // p.restart
+
+
+# relative agreement of the residual histories: fp64 storage reproduces the oracle to rounding; with
+# reduced storage a rounding-level difference in w can move an entry of v across a rounding boundary
+# of the format at the store, a perturbation of one unit of the format's precision
+HIST_TOL = {"fp64": 1e-12, "fp32": 2.0 ** -24, "fp16": 2.0 ** -11, "int32": 1.0 / 2147483647, "int16": 1.0 / 32767}
+
+
+@pytest.mark.parametrize("fmt", oracle.FORMATS)
+def test_full_size_c2_residual_history_prefix(c2_full, fmt):
+    """Bounded prefix of the full-size solve against the oracle: the recurrence residual of the first
+    40 Arnoldi steps (one step = SpMV + both Gram-Schmidt passes + store at n = 1e6) and the
+    re-orthogonalisation decisions (reading Q11: the iterates differ by summation order only)."""
+    p, s = c2_full
+    steps = 40
+    ref = oracle.gmres(p.A, p.b, p.x0, p.restart, p.rel_tol, steps, fmt=fmt)
+    _, r = s.solve(p.b, p.x0, p.restart, p.rel_tol, steps, fmt, history=True)
+    assert r.iters == ref.iters == steps
+    hg, ho = np.asarray(r.rec_history[:steps]), np.asarray(ref.rec_history[:steps])
+    assert np.all(np.abs(hg - ho) <= HIST_TOL[fmt] * ho)
+    assert r.reorth_count == ref.reorth_count
