@@ -421,7 +421,44 @@ template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_
                         e[u] = rowptr(row + 1);
                     }
                 }
+                // The index and value arrays of a block lie wholly inside the staged (16-byte aligned) part of
+                // the matrix except in the last block(s) of the matrix: a block-uniform flag picks the loop
+                // whose guards are predicates on shared-memory loads (no divergence, ~10 instructions per
+                // nonzero) and keeps the per-element shared/global select for that tail only.
+                const bool tail_blk = p1 > safe_ci || p1 > safe_va;
                 bool more = true;
+                if (!tail_blk) {
+                    const int32_t *sci = st.ci + oc;
+                    const double *sva = st.va + ov;
+                    while (more) {
+                        int c[RPT][KU];
+#pragma unroll
+                        for (int u = 0; u < RPT; ++u)
+#pragma unroll
+                            for (int k = 0; k < KU; ++k) {
+                                const int g = q[u] + k * LPR;
+                                c[u][k] = (g < e[u]) ? sci[g] : 0;
+                            }
+                        double xv[RPT][KU];
+#pragma unroll
+                        for (int u = 0; u < RPT; ++u)
+#pragma unroll
+                            for (int k = 0; k < KU; ++k) xv[u][k] = __ldg(x + c[u][k]);
+                        more = false;
+#pragma unroll
+                        for (int u = 0; u < RPT; ++u) {
+#pragma unroll
+                            for (int k = 0; k < KU; ++k) {
+                                const int g = q[u] + k * LPR;
+                                const double av = (g < e[u]) ? sva[g] : 0.0;
+                                s[u] = fma(av, xv[u][k], s[u]);
+                            }
+                            q[u] += KU * LPR;
+                            more |= q[u] < e[u];
+                        }
+                        more = __any_sync(0xffffffffu, more);
+                    }
+                }
                 while (more) {
                     int c[RPT][KU];
 #pragma unroll
@@ -450,9 +487,12 @@ template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_
                     }
                     more = __any_sync(0xffffffffu, more);
                 }
-                __threadfence_block(); // the stage's loads must have completed, not merely been issued
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&sm.empty[ring.s]);
+                { // hand the stage back once its loads have been USED (device_utils.cuh): the sums depend on all of them
+                    unsigned dep = 0;
+#pragma unroll
+                    for (int u = 0; u < RPT; ++u) dep ^= dep_bits(s[u]);
+                    mbar_arrive_after_use(&sm.empty[ring.s], lane, dep);
+                }
 #pragma unroll
                 for (int u = 0; u < RPT; ++u) {
 #pragma unroll
