@@ -298,6 +298,16 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src, uint32
                  : "memory");
 }
 
+// The same with an L2 cache policy (createpolicy): the matrix stream of the SpMV is marked evict-first so
+// that it does not push the basis and the vectors out of the 126 MB L2 between two Gram-Schmidt passes.
+__device__ __forceinline__ void bulk_g2s_hint(void *dst_smem, const void *src, uint32_t bytes, uint64_t *bar, uint64_t policy)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+                 : "memory");
+}
+
 // ---- programmatic dependent launch ------------------------------------------------------------------
 // The kernels of an Arnoldi step form a chain on one stream, each 10-100 us long.  Launched with
 // the programmatic-stream-serialisation attribute, the next kernel's CTAs are scheduled while the

@@ -376,6 +376,7 @@ template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_
     if (warp == kRowsThreads / 32) {
         // ---- producer ----------------------------------------------------------------------------------
         Ring ring;
+        const uint64_t pol = policy_evict_first(); // the matrix is read once per step: keep the L2 for basis and vectors
         int np0 = 0, np1 = 0;
         if ((int)blockIdx.x < nblk) {
             np0 = rp[blockIdx.x * RB];
@@ -398,8 +399,8 @@ template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_
                     bytes_va = (uint32_t)max(0, min((p1 + 1) & ~1, safe_va) - pv) * 8u;
                 }
                 mbar_expect_tx(&sm.full[ring.s], bytes_ci + bytes_va + bytes_rp);
-                if (bytes_ci) bulk_g2s(st.ci, ci + pc, bytes_ci, &sm.full[ring.s]);
-                if (bytes_va) bulk_g2s(st.va, va + pv, bytes_va, &sm.full[ring.s]);
+                if (bytes_ci) bulk_g2s_hint(st.ci, ci + pc, bytes_ci, &sm.full[ring.s], pol);
+                if (bytes_va) bulk_g2s_hint(st.va, va + pv, bytes_va, &sm.full[ring.s], pol);
                 if (bytes_rp) bulk_g2s(st.rp, rp + ra, bytes_rp, &sm.full[ring.s]);
             }
             __syncwarp();
