@@ -78,6 +78,7 @@ struct OrthArgs {
     int last_range;       // UPD kinds: the finaliser of this launch publishes the norms
     int nstages;
     int interleave;       // row tiles dealt round-robin to the CTAs (else one contiguous row range per CTA)
+    int dir;              // 1: walk the row tiles from the last to the first
 };
 
 // 2D tiled TMA copy global -> shared: box [box0 8-byte elements x 8 columns] at element (x, y) of
@@ -489,22 +490,6 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
     constexpr bool HAS_UPD = KIND != PASS_DOT, HAS_DOT = KIND != PASS_UPD;
     Ctl *ctl = a.ctl;
     if (threadIdx.x == 0) TR(0);
-    pdl_wait();
-    pdl_launch_dependents();
-    if (threadIdx.x == 0) TR(1);
-    // the control words this CTA needs, fetched together (each is an L2 round trip)
-    const int stop_after = __ldcg(&ctl->stop_after), reorth_flag = __ldcg(&ctl->reorth_flag), ctl_dir = __ldcg(&ctl->dir);
-    const int dk = a.d_k ? __ldcg(a.d_k) : 0;
-    if (a.mode == MODE_ORTH1 || a.mode == MODE_ORTH2) {
-        if (a.step > stop_after) return;
-        if (a.mode == MODE_ORTH2 && !reorth_flag) return;
-    }
-    int k = a.k;
-    if (a.d_k) { // cycle-end x update: the number of basis vectors is only known on the device
-        k = min(a.k, dk - a.c0);
-        if (k <= 0) return;
-    }
-    const int nst = (k + T::STAGE_COLS - 1) / T::STAGE_COLS; // stages per row tile
     const int ns = a.nstages;
 
     extern __shared__ __align__(128) unsigned char smem[];
@@ -530,14 +515,11 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (HAS_UPD)
-        for (int c = tid; c < kMaxRangeCols; c += kOrthThreads) hs_s[c] = (c < k) ? a.hs[c] * T::Fm::PRE : 0.0;
     __syncthreads();
 
-    // Row tiles of this CTA.  Blocked: one contiguous row range per CTA (a multiple of 64 rows, so
-    // every tile start is 16-byte aligned in every format), perfectly balanced whatever the tile
-    // height.  Interleaved: tile t belongs to CTA t mod grid, so the CTAs sweep a contiguous window
-    // of the basis together and short column segments still arrive at the DRAM as long runs.
+    // Row tiles of this CTA.  Interleaved (default): tile t belongs to CTA t mod grid, so the CTAs
+    // sweep a contiguous window of the basis together.  Blocked: one contiguous row range per CTA (a
+    // multiple of 64 rows, so every tile start is 16-byte aligned in every format).
     int64_t row_begin, row_end, tile_stride;
     int ntiles;
     if (a.interleave) {
@@ -554,7 +536,61 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
         ntiles = (int)((row_end - row_begin + R - 1) / R);
         tile_stride = R;
     }
-    const int dir = (a.mode == MODE_HOOK) ? 0 : ctl_dir; // consecutive passes walk in opposite directions
+    const int dir = a.dir; // consecutive passes of a step walk in opposite directions (set by the host)
+
+    // One stage of row tile (first row r0) into ring slot `slot`: lane 0 arms the barrier, lanes 0..3 issue the boxes.
+    auto issue_stage = [&](int64_t r0, int st, int slot, int kk) {
+        const int x0 = (int)(r0 * B / 8); // first 8-byte word of the tile inside a column
+        const int c_first = st * T::STAGE_COLS;
+        // boxes of this stage that hold at least one wanted column (F = 4: both halves of 8 columns)
+        const int nboxes = (F == 4) ? T::BOXES : min(T::BOXES, (kk - c_first + kChunkCols - 1) / kChunkCols);
+        if (lane == 0) mbar_expect_tx(&full[slot], nboxes * T::BOX_BYTES);
+        __syncwarp();
+        if (lane < nboxes) {
+            unsigned char *dst = stages + (size_t)slot * T::STAGE + lane * T::BOX_BYTES;
+            if (F == 4) tma_box_g2s(dst, &tmap, x0 + lane * (T::BOX_INNER / 8), c_first, &full[slot]);
+            else tma_box_g2s(dst, &tmap, x0, c_first + lane * kChunkCols, &full[slot]);
+        }
+    };
+
+    // ---- before the grid dependency resolves: the basis is not written by the predecessor kernel (the
+    // store of the newest vector completed before the predecessor started), so the producer already
+    // fetches the first stages of the first row tile while the predecessor's tail -- its last CTAs and
+    // the last-block-done final stage -- is still running.  Nothing else is read before the wait.
+    int pre = 0;
+    if (warp == kConsumerWarps && !a.d_k && ntiles > 0) {
+        const int nst0 = (a.k + T::STAGE_COLS - 1) / T::STAGE_COLS;
+        pre = nst0 < ns ? nst0 : ns;
+        const int t0 = dir ? ntiles - 1 : 0;
+        for (int st = 0; st < pre; ++st) issue_stage(row_begin + (int64_t)t0 * tile_stride, st, st, a.k);
+        if (lane == 0) TR(30);
+    }
+    pdl_wait();
+    pdl_launch_dependents();
+    if (threadIdx.x == 0) TR(1);
+    // the control words this CTA needs, fetched together (each is an L2 round trip)
+    const int stop_after = __ldcg(&ctl->stop_after), reorth_flag = __ldcg(&ctl->reorth_flag);
+    const int dk = a.d_k ? __ldcg(a.d_k) : 0;
+    int k = a.k;
+    bool run = true;
+    if (a.mode == MODE_ORTH1 || a.mode == MODE_ORTH2) {
+        if (a.step > stop_after) run = false;
+        if (a.mode == MODE_ORTH2 && !reorth_flag) run = false;
+    }
+    if (a.d_k) { // cycle-end x update: the number of basis vectors is only known on the device
+        k = min(a.k, dk - a.c0);
+        if (k <= 0) run = false;
+    }
+    if (!run) { // copies in flight must land before the CTA gives its shared memory back
+        if (warp == kConsumerWarps && lane == 0)
+            for (int s = 0; s < pre; ++s) mbar_wait(&full[s], 0u);
+        return;
+    }
+    const int nst = (k + T::STAGE_COLS - 1) / T::STAGE_COLS; // stages per row tile
+    if (HAS_UPD && tid < kConsumers) {
+        for (int c = tid; c < kMaxRangeCols; c += kConsumers) hs_s[c] = (c < k) ? a.hs[c] * T::Fm::PRE : 0.0;
+        consumer_bar();
+    }
     if (threadIdx.x == 0) TR(2);
 
     double acc[kMaxChunks];
@@ -580,21 +616,10 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
                     tma_box_g2s(wbuf + wslot * R, &wmap, 0, (int)(r0 / T::VEC), &wfull[wslot]);
                 }
             }
-            const int x0 = (int)(r0 * B / 8); // first 8-byte word of the tile inside a column
             for (int st = 0; st < nst; ++st) {
-                const int c_first = st * T::STAGE_COLS;
-                // boxes of this stage that hold at least one wanted column (F = 4: both halves of 8 columns)
-                const int nboxes = (F == 4) ? T::BOXES : min(T::BOXES, (k - c_first + kChunkCols - 1) / kChunkCols);
-                if (lane == 0) {
-                    mbar_wait(&empty[ring.s], ring.ph ^ 1u);
-                    mbar_expect_tx(&full[ring.s], nboxes * T::BOX_BYTES);
-                }
-                __syncwarp();
-                if (lane == 0 && i == 0 && st == 0) TR(30);
-                if (lane < nboxes) {
-                    unsigned char *dst = stages + (size_t)ring.s * T::STAGE + lane * T::BOX_BYTES;
-                    if (F == 4) tma_box_g2s(dst, &tmap, x0 + lane * (T::BOX_INNER / 8), c_first, &full[ring.s]);
-                    else tma_box_g2s(dst, &tmap, x0, c_first + lane * kChunkCols, &full[ring.s]);
+                if (i > 0 || st >= pre) { // (the first `pre` stages of the first tile are already on their way)
+                    if (lane == 0) mbar_wait(&empty[ring.s], ring.ph ^ 1u);
+                    issue_stage(r0, st, ring.s, k);
                 }
                 ring.advance(ns);
             }
@@ -685,7 +710,7 @@ int choose_seg_kb(int format, int kind, int k, int64_t n, int forced)
     return 0;
 }
 
-int g_interleave_opt = 0; // 0 = interleave the short segments (1-2 KB), 1 = never, 2 = always
+int g_interleave_opt = 0; // 0 = auto (interleave), 1 = never (one contiguous row range per CTA), 2 = always
 int g_orth_error = 0;     // CUresult of the last failed tensor-map encode (0 = none)
 
 // ---- tensor maps: the basis as a 2D array [k columns][ceil(n*B/8) 8-byte words], box = 8 columns x
@@ -793,7 +818,7 @@ const CUtensorMap *w_map(const double *w, int64_t n, int vec, int R)
 template <int FMT, int F, int KIND> int launch_inst(cudaStream_t s, OrthArgs &a)
 {
     using T = Tile<FMT, F>;
-    a.interleave = g_interleave_opt == 2 || (g_interleave_opt == 0 && F <= 2);
+    a.interleave = g_interleave_opt != 1; // measured: the shared sliding window wins for every segment size (fp64 k = 100: 6.46 -> 6.75 TB/s)
     static bool attr_set = false;
     if (!attr_set) {
         cudaFuncSetAttribute(orth_kernel<FMT, F, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, kOrthSmemBytes);
@@ -882,6 +907,7 @@ int launch_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b, int64
     for (int c0 = 0; c0 < k; c0 += kMaxRangeCols) {
         const int kk = (k - c0 < kMaxRangeCols) ? k - c0 : kMaxRangeCols;
         OrthArgs a = base_args(sc, b, n, mode, step);
+        a.dir = 0; // dot forwards, first update backwards, second update forwards: each pass starts where the previous one ended
         a.V = static_cast<const char *>(b.V) + (int64_t)c0 * col_bytes;
         a.scales = b.scales ? b.scales + c0 : nullptr;
         a.w = const_cast<double *>(w);
@@ -903,6 +929,7 @@ int launch_update(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t
     for (int c0 = 0; c0 < k; c0 += kMaxRangeCols) {
         const int kk = (k - c0 < kMaxRangeCols) ? k - c0 : kMaxRangeCols;
         OrthArgs a = base_args(sc, b, n, mode, step);
+        a.dir = (mode == MODE_ORTH1) ? 1 : 0; // dot forwards, first update backwards, second update forwards: each pass starts where the previous one ended
         a.V = static_cast<const char *>(b.V) + (int64_t)c0 * col_bytes;
         a.hs = hs + c0;
         a.d_k = d_k;
@@ -925,6 +952,7 @@ int launch_update_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b
 {
     if (!update_multidot_fits(b.format, k, seg_kb)) return 0;
     OrthArgs a = base_args(sc, b, n, mode, step);
+        a.dir = (mode == MODE_HOOK) ? 0 : 1; // dot forwards, first update backwards, second update forwards: each pass starts where the previous one ended
     a.hs = hs;
     a.w = w;
     a.k = k;

@@ -348,9 +348,10 @@ struct RowsSmem {
 
 template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_rows_kernel(const SpmvArgs a)
 {
-    pdl_wait();
-    pdl_launch_dependents();
-    if (a.mode == MODE_STEP && a.step > a.ctl->stop_after) return;
+    // The matrix is never written by a predecessor kernel: the producer warp fetches its first
+    // blocks BEFORE the grid dependency resolves (while the predecessor's tail is still running);
+    // everything else -- x, the control block -- is read after the wait.
+    const bool is_producer = (threadIdx.x >> 5) == kRowsThreads / 32;
     constexpr int RB = kRowsThreads * RPT / LPR, KU = kRowsGathers / RPT, RSTRIDE = kRowsThreads / LPR;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     RowsSmem &sm = *reinterpret_cast<RowsSmem *>(smem_raw);
@@ -370,6 +371,11 @@ template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    if (!is_producer) {
+        pdl_wait();
+        pdl_launch_dependents();
+        if (a.mode == MODE_STEP && a.step > a.ctl->stop_after) return;
+    }
     double ss = 0.0, am = 0.0;
     const int nblk = (n + RB - 1) / RB, stride = gridDim.x;
 
@@ -382,7 +388,21 @@ template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_
             np0 = rp[blockIdx.x * RB];
             np1 = rp[min(n, (int)(blockIdx.x + 1) * RB)];
         }
+        int issued = 0;
+        bool waited = false;
+        auto dependency = [&]() { // returns false if this step is skipped: drain the copies in flight and leave
+            pdl_wait();
+            pdl_launch_dependents();
+            waited = true;
+            if (a.mode == MODE_STEP && a.step > a.ctl->stop_after) {
+                if (lane == 0)
+                    for (int s2 = 0; s2 < issued; ++s2) mbar_wait(&sm.full[s2], 0u);
+                return false;
+            }
+            return true;
+        };
         for (int blk = blockIdx.x; blk < nblk; blk += stride) {
+            if (!waited && issued == kRowsStages && !dependency()) return;
             const int r0 = blk * RB, r1 = min(n, r0 + RB), p0 = np0, p1 = np1;
             if (blk + stride < nblk) { // row pointers of the next block, one iteration ahead
                 np0 = rp[(blk + stride) * RB];
@@ -405,7 +425,9 @@ template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_
             }
             __syncwarp();
             ring.advance(kRowsStages);
+            ++issued;
         }
+        if (!waited && !dependency()) return;
     } else {
         // ---- consumers: lane group tid / LPR owns rows r0 + tid / LPR + u * RSTRIDE of the block ----------
         const int gl = tid % LPR;

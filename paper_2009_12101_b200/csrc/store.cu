@@ -91,7 +91,10 @@ template <int FMT, int THREADS> __global__ void __launch_bounds__(THREADS) store
     using F = Fmt<FMT>;
     constexpr int VEC = F::VEC;
     pdl_wait();
-    pdl_launch_dependents();
+    // A successor may fetch basis columns before ITS grid dependency resolves (orth.cu); inside a solve
+    // the successor of a store is never a Gram-Schmidt pass, but after the k_compress / k_store hooks it
+    // can be: there the successor is only released when this kernel has completed.
+    if (a.mode != MODE_HOOK) pdl_launch_dependents();
     // control words fetched together (each is an L2 round trip)
     const int stop_after = (a.mode != MODE_HOOK) ? __ldcg(&a.ctl->stop_after) : 0;
     const double hn_dev = a.d_hn ? __ldcg(a.d_hn) : 0.0, amax_dev = a.d_amax ? __ldcg(a.d_amax) : 0.0;
