@@ -571,6 +571,8 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
     // the control words this CTA needs, fetched together (each is an L2 round trip)
     const int stop_after = __ldcg(&ctl->stop_after), reorth_flag = __ldcg(&ctl->reorth_flag);
     const int dk = a.d_k ? __ldcg(a.d_k) : 0;
+    double hs_v = 0.0; // this thread's update coefficient, fetched in the same round trip as the control words
+    if (HAS_UPD && tid < a.k) hs_v = __ldcg(&a.hs[tid]);
     int k = a.k;
     bool run = true;
     if (a.mode == MODE_ORTH1 || a.mode == MODE_ORTH2) {
@@ -588,7 +590,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
     }
     const int nst = (k + T::STAGE_COLS - 1) / T::STAGE_COLS; // stages per row tile
     if (HAS_UPD && tid < kConsumers) {
-        for (int c = tid; c < kMaxRangeCols; c += kConsumers) hs_s[c] = (c < k) ? a.hs[c] * T::Fm::PRE : 0.0;
+        if (tid < kMaxRangeCols) hs_s[tid] = (tid < k) ? hs_v * T::Fm::PRE : 0.0;
         consumer_bar();
     }
     if (threadIdx.x == 0) TR(2);

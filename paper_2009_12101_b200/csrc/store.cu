@@ -95,7 +95,17 @@ template <int FMT, int THREADS> __global__ void __launch_bounds__(THREADS) store
     // the successor of a store is never a Gram-Schmidt pass, but after the k_compress / k_store hooks it
     // can be: there the successor is only released when this kernel has completed.
     if (a.mode != MODE_HOOK) pdl_launch_dependents();
-    // control words fetched together (each is an L2 round trip)
+    // this thread's first rows of w and the control words, fetched together (each is an L2 round trip)
+    const bool has_ctl_cta0 = a.has_cyc && a.mode == MODE_ORTH1;
+    const int bid0 = has_ctl_cta0 ? (int)blockIdx.x - 1 : (int)blockIdx.x;
+    const int nblk = has_ctl_cta0 ? gridDim.x - 1 : gridDim.x;
+    const int64_t ngroups = (a.n + VEC - 1) / VEC;
+    const int64_t g0 = (int64_t)bid0 * THREADS + threadIdx.x;
+    double2 w0[VEC / 2];
+    if (bid0 >= 0 && g0 < ngroups && g0 * VEC + VEC <= a.n) {
+#pragma unroll
+        for (int r = 0; r < VEC; r += 2) w0[r / 2] = *reinterpret_cast<const double2 *>(a.w + g0 * VEC + r);
+    }
     const int stop_after = (a.mode != MODE_HOOK) ? __ldcg(&a.ctl->stop_after) : 0;
     const double hn_dev = a.d_hn ? __ldcg(a.d_hn) : 0.0, amax_dev = a.d_amax ? __ldcg(a.d_amax) : 0.0;
     if (a.mode != MODE_HOOK && a.step > stop_after) return;
@@ -123,15 +133,13 @@ template <int FMT, int THREADS> __global__ void __launch_bounds__(THREADS) store
     }
     if (bid == 0 && threadIdx.x == 0) *a.scale_out = sigma;
 
-    const int nblk = has_ctl_cta ? gridDim.x - 1 : gridDim.x;
-    const int64_t ngroups = (a.n + VEC - 1) / VEC;
-    for (int64_t g = (int64_t)bid * THREADS + threadIdx.x; g < ngroups; g += (int64_t)nblk * THREADS) {
+    for (int64_t g = g0; g < ngroups; g += (int64_t)nblk * THREADS) {
         const int64_t row = g * VEC;
         if (row + VEC <= a.n) {
             double v[VEC];
 #pragma unroll
             for (int r = 0; r < VEC; r += 2) {
-                const double2 t = *reinterpret_cast<const double2 *>(a.w + row + r);
+                const double2 t = (g == g0) ? w0[r / 2] : *reinterpret_cast<const double2 *>(a.w + row + r);
                 v[r] = t.x / hn; // IEEE division per element (reading Q8)
                 v[r + 1] = t.y / hn;
             }
