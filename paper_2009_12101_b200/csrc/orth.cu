@@ -205,13 +205,12 @@ __device__ __forceinline__ void for_valid_chunks(int nv, const unsigned char *st
 // therefore stored with the TMA 32-byte / 64-byte swizzle (16-byte chunk index XOR address bits
 // 7.. ), which spreads the lanes of a quarter warp over all eight 16-byte bank groups.  fp64
 // (16 bytes of w per word) needs none.
-template <int VEC> __device__ __forceinline__ double *wswz(double *p)
+template <int VEC> __device__ __forceinline__ int wswz(uint32_t base_saddr, int idx) // idx: row of the tile at shared address base_saddr
 {
-    if constexpr (VEC == 2) return p;
-    const uintptr_t a = reinterpret_cast<uintptr_t>(p);
-    return reinterpret_cast<double *>(a ^ (((a >> 7) & (VEC == 8 ? 3u : 1u)) << 4));
+    if constexpr (VEC == 2) return idx;
+    const uint32_t a = base_saddr + (uint32_t)idx * 8u;
+    return idx ^ (int)(((a >> 7) & (VEC == 8 ? 3u : 1u)) << 1); // 16-byte chunk index XOR address bits 7..: two doubles per chunk
 }
-template <int VEC> __device__ __forceinline__ const double *wswz(const double *p) { return wswz<VEC>(const_cast<double *>(p)); }
 
 struct ConsumerCtx {
     uint64_t *full, *empty, *wfull, *wempty;
@@ -234,6 +233,7 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
     constexpr bool HAS_UPD = KIND != PASS_DOT, HAS_DOT = KIND != PASS_UPD;
     const int wi0 = c.half * T::WORDS_HALF + c.lane; // this lane's first 16-byte word in a column segment
     double *wt = c.wbuf + wslot * R;
+    const uint32_t wt_s = smem_u32(wt), red_s = smem_u32(c.red), w1_s = smem_u32(c.w1buf);
 
     mbar_wait(&c.wfull[wslot], wph);
     if (RAGGED) {
@@ -243,19 +243,20 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
         } else { // 2D box over complete groups of VEC rows (beyond them: zero fill); the last n % VEC rows by hand
             const int64_t nfull = a.n / VEC * VEC;
             if (r0 + rows == a.n && nfull < a.n)
-                for (int r = (int)(nfull - r0) + c.ct; r < rows; r += kConsumers) *wswz<VEC>(wt + r) = a.w[r0 + r];
+                for (int r = (int)(nfull - r0) + c.ct; r < rows; r += kConsumers) wt[wswz<VEC>(wt_s, r)] = a.w[r0 + r];
             if (nfull == 0) // n < VEC: the map's single group is in range although incomplete
-                for (int r = rows + c.ct; r < VEC; r += kConsumers) *wswz<VEC>(wt + r) = 0.0;
+                for (int r = rows + c.ct; r < VEC; r += kConsumers) wt[wswz<VEC>(wt_s, r)] = 0.0;
         }
         consumer_bar();
     }
     // rows of w owned by this lane, pre-multiplied by PRE (see "widening" in device_utils.cuh)
     auto load_w = [&](const double *src, double (&wreg)[GV]) {
+        const uint32_t src_s = smem_u32(src);
 #pragma unroll
         for (int f = 0; f < F; ++f)
 #pragma unroll
             for (int v = 0; v < VEC; v += 2) {
-                const double2 t = *reinterpret_cast<const double2 *>(wswz<VEC>(src + (wi0 + f * 32) * VEC + v));
+                const double2 t = *reinterpret_cast<const double2 *>(src + wswz<VEC>(src_s, (wi0 + f * 32) * VEC + v));
                 wreg[f * VEC + v] = (PRE == 1.0) ? t.x : t.x * PRE;
                 wreg[f * VEC + v + 1] = (PRE == 1.0) ? t.y : t.y * PRE;
             }
@@ -329,18 +330,19 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
         ring.advance(c.ns);
     }
     double *redw = c.red + c.cw * R;
+    const uint32_t redw_s = smem_u32(redw);
 #pragma unroll
     for (int f = 0; f < F; ++f)
 #pragma unroll
         for (int v = 0; v < VEC; v += 2)
-            *reinterpret_cast<double2 *>(wswz<VEC>(redw + (wi0 + f * 32) * VEC + v)) = make_double2(p[f * VEC + v], p[f * VEC + v + 1]);
+            *reinterpret_cast<double2 *>(redw + wswz<VEC>(redw_s, (wi0 + f * 32) * VEC + v)) = make_double2(p[f * VEC + v], p[f * VEC + v + 1]);
     consumer_bar();
     // new w of the tile: the eight partial row vectors are added in a fixed order
     for (int r = c.ct; r < R; r += kConsumers) {
         double tot = 0.0;
 #pragma unroll
-        for (int q = 0; q < kColWarps; ++q) tot += *wswz<VEC>(c.red + q * R + r); // stored like the w tiles: conflict-free both ways
-        const double wo = *wswz<VEC>(wt + r);
+        for (int q = 0; q < kColWarps; ++q) tot += c.red[q * R + wswz<VEC>(red_s + q * R * 8, r)]; // stored like the w tiles: conflict-free both ways
+        const double wo = wt[wswz<VEC>(wt_s, r)];
         const double wn = (PRE == 1.0) ? wo - tot : fma(-tot, PRE, wo); // tot * PRE is exact: one rounding either way
         const bool live = !RAGGED || r < rows;
         if (live) {
@@ -348,7 +350,7 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
             ss = fma(wn, wn, ss);
             am = fmax(am, fabs(wn));
         }
-        if (HAS_DOT) *wswz<VEC>(c.w1buf + r) = live ? wn : 0.0; // kept apart from the TMA-written slot: no proxy fence
+        if (HAS_DOT) c.w1buf[wswz<VEC>(w1_s, r)] = live ? wn : 0.0; // kept apart from the TMA-written slot: no proxy fence
     }
     consumer_bar();
     release_w(dep_bits(ss)); // the tile of w was consumed by the stores of the new w and by the norms
@@ -707,7 +709,10 @@ int choose_seg_kb(int format, int kind, int k, int64_t n, int forced)
     }
     for (int f = fmax; f >= 1; f >>= 1) {
         if (!feasible(f)) continue;
-        if (f == 1 || (int64_t)f * 1024 / B * 2 <= per) return f; // at least two full tiles per CTA
+        // at least twelve row tiles per CTA: with fewer, pipeline ramp, tail and the one-tile imbalance of the
+        // round-robin deal show (C2, n = 1e6, us per Arnoldi step at 6.6 / 13 / 26 tiles per CTA: fp32 182 / 169 / 172,
+        // fp16 150 / 141 / -)
+        if (f == 1 || (int64_t)f * 1024 / B * 12 <= per) return f;
     }
     return 0;
 }
