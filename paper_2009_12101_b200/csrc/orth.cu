@@ -212,6 +212,81 @@ template <int VEC> __device__ __forceinline__ int wswz(uint32_t base_saddr, int 
     return idx ^ (int)(((a >> 7) & (VEC == 8 ? 3u : 1u)) << 1); // 16-byte chunk index XOR address bits 7..: two doubles per chunk
 }
 
+// ---- row-owner mapping of the update -----------------------------------------------------------------
+// Each of the 512 consumer threads owns SEG / 512 = 2 F bytes of every column segment -- one or two
+// whole entries when 2 F >= B -- i.e. its own rows of the tile: the sum over ALL columns stays in the
+// thread (no partial row vectors through shared memory, no CTA barrier for the reduction), every
+// thread works on every column whatever k is, and the new w leaves the thread that computed it.
+// Entries go through the conversion pipe here (one instruction each; true values, unscaled
+// coefficients); the dot sweeps keep the integer widening.
+// Used for the plain update and for the fused kind with fp64 storage; the fused kind with reduced
+// storage is faster with the column mapping (measured, fp16 k = 100, n = 4.2e6: 261 vs 289 us -- one
+// 2-byte shared-memory load per entry costs more than the reduction it saves).
+template <int FMT, int F, int KIND> __host__ __device__ constexpr bool upd_rowmap()
+{
+    return 2 * F >= Fmt<FMT>::BYTES && (KIND == PASS_UPD || FMT == CBGMRES_FP64);
+}
+
+__device__ __forceinline__ void half2_cvt(unsigned w, double &lo, double &hi) // F2F.F64.F16 takes either half of a register
+{
+    asm("{.reg .b16 l, h; mov.b32 {l, h}, %2; cvt.f64.f16 %0, l; cvt.f64.f16 %1, h;}" : "=d"(lo), "=d"(hi) : "r"(w));
+}
+__device__ __forceinline__ void i16x2_cvt(unsigned w, double &lo, double &hi)
+{
+    asm("{.reg .b16 l, h; mov.b32 {l, h}, %2; cvt.rn.f64.s16 %0, l; cvt.rn.f64.s16 %1, h;}" : "=d"(lo), "=d"(hi) : "r"(w));
+}
+template <int FMT, int UB> struct Unit; // UB payload bytes -> EU = UB / B doubles
+template <> struct Unit<CBGMRES_FP64, 8> {
+    static constexpr int EU = 1;
+    static __device__ __forceinline__ void load(const unsigned char *p, double (&d)[1]) { d[0] = *reinterpret_cast<const double *>(p); }
+};
+template <> struct Unit<CBGMRES_FP32, 4> {
+    static constexpr int EU = 1;
+    static __device__ __forceinline__ void load(const unsigned char *p, double (&d)[1]) { d[0] = (double)*reinterpret_cast<const float *>(p); }
+};
+template <> struct Unit<CBGMRES_FP32, 8> {
+    static constexpr int EU = 2;
+    static __device__ __forceinline__ void load(const unsigned char *p, double (&d)[2])
+    {
+        const float2 f = *reinterpret_cast<const float2 *>(p);
+        d[0] = (double)f.x;
+        d[1] = (double)f.y;
+    }
+};
+template <> struct Unit<CBGMRES_INT32, 4> {
+    static constexpr int EU = 1;
+    static __device__ __forceinline__ void load(const unsigned char *p, double (&d)[1]) { d[0] = (double)*reinterpret_cast<const int *>(p); }
+};
+template <> struct Unit<CBGMRES_INT32, 8> {
+    static constexpr int EU = 2;
+    static __device__ __forceinline__ void load(const unsigned char *p, double (&d)[2])
+    {
+        const int2 q = *reinterpret_cast<const int2 *>(p);
+        d[0] = (double)q.x;
+        d[1] = (double)q.y;
+    }
+};
+template <> struct Unit<CBGMRES_FP16, 2> {
+    static constexpr int EU = 1;
+    static __device__ __forceinline__ void load(const unsigned char *p, double (&d)[1])
+    {
+        const unsigned short h = *reinterpret_cast<const unsigned short *>(p);
+        asm("cvt.f64.f16 %0, %1;" : "=d"(d[0]) : "h"(h));
+    }
+};
+template <> struct Unit<CBGMRES_FP16, 4> {
+    static constexpr int EU = 2;
+    static __device__ __forceinline__ void load(const unsigned char *p, double (&d)[2]) { half2_cvt(*reinterpret_cast<const unsigned *>(p), d[0], d[1]); }
+};
+template <> struct Unit<CBGMRES_INT16, 2> {
+    static constexpr int EU = 1;
+    static __device__ __forceinline__ void load(const unsigned char *p, double (&d)[1]) { d[0] = (double)*reinterpret_cast<const short *>(p); }
+};
+template <> struct Unit<CBGMRES_INT16, 4> {
+    static constexpr int EU = 2;
+    static __device__ __forceinline__ void load(const unsigned char *p, double (&d)[2]) { i16x2_cvt(*reinterpret_cast<const unsigned *>(p), d[0], d[1]); }
+};
+
 struct ConsumerCtx {
     uint64_t *full, *empty, *wfull, *wempty;
     const double *hs_s;
@@ -306,8 +381,79 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
         return;
     }
 
-    // ---- update: p = sum_c dec(V)[rows, c] * hs_c over this warp's columns (hs_s holds PRE * hs_c) ------
     const Ring tile_start = ring;
+    if constexpr (upd_rowmap<FMT, F, KIND>()) {
+        // ---- update, row-owner mapping: this thread's rows, all columns (hs_s holds hs_c unscaled) -----------
+        constexpr int UB = 2 * F;
+        using U = Unit<FMT, UB>;
+        constexpr int EU = U::EU;
+        // byte offset of this thread's unit inside a column segment of the stage layout (word_ptr)
+        const int ub = c.ct * UB;
+        const int uoff = (F == 4) ? (ub >> 11) * T::BOX_BYTES + (ub & 2047) : ub;
+        constexpr int CSTR = (F == 4) ? T::BOX_INNER : T::SEG; // distance between columns of a stage
+        double pa[EU], pb[EU]; // two chains (even / odd columns)
+#pragma unroll
+        for (int e = 0; e < EU; ++e) pa[e] = pb[e] = 0.0;
+        for (int st = 0; st < c.nst; ++st) {
+            const int c0s = st * T::STAGE_COLS;
+            const int nc = min(T::STAGE_COLS, c.k - c0s); // columns of this stage that exist (the rest may be stale memory)
+            mbar_wait(&c.full[ring.s], ring.ph);
+            const unsigned char *base = c.stages + (size_t)ring.s * T::STAGE + uoff;
+            int lc = 0;
+            for (; lc + 8 <= nc; lc += 8) { // eight columns at a time: all loads first
+                double d[8][EU];
+                double2 cf[4];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) U::load(base + (lc + j) * CSTR, d[j]);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) cf[j] = *reinterpret_cast<const double2 *>(c.hs_s + c0s + lc + 2 * j);
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+#pragma unroll
+                    for (int e = 0; e < EU; ++e) {
+                        pa[e] = fma(d[2 * j][e], cf[j].x, pa[e]);
+                        pb[e] = fma(d[2 * j + 1][e], cf[j].y, pb[e]);
+                    }
+            }
+            for (; lc < nc; ++lc) {
+                double d[EU];
+                U::load(base + lc * CSTR, d);
+                const double cf = c.hs_s[c0s + lc];
+#pragma unroll
+                for (int e = 0; e < EU; ++e) pa[e] = fma(d[e], cf, pa[e]);
+            }
+            if (KIND == PASS_UPD) release_stage(ring.s, dep_bits(pa[0]) ^ dep_bits(pb[0]));
+            ring.advance(c.ns);
+        }
+        // new w of this thread's rows.  Two buffers for the second sweep, alternating by tile: no barrier
+        // separates a fast thread's writes for this tile from a slow thread's reads of the previous one
+        // (the unused `red` area is the second buffer).
+        double *w1 = (wslot & 1) ? c.red : c.w1buf;
+        const uint32_t w1r_s = smem_u32(w1);
+        const int rbase = c.ct * EU;
+        double wn[EU];
+#pragma unroll
+        for (int e = 0; e < EU; ++e) {
+            const int r = rbase + e;
+            wn[e] = wt[wswz<VEC>(wt_s, r)] - (pa[e] + pb[e]);
+            const bool live = !RAGGED || r < rows;
+            if (live) {
+                ss = fma(wn[e], wn[e], ss);
+                am = fmax(am, fabs(wn[e]));
+            } else wn[e] = 0.0;
+            if (HAS_DOT) w1[wswz<VEC>(w1r_s, r)] = wn[e]; // kept apart from the TMA-written slot: no proxy fence
+        }
+        if (EU == 2 && (!RAGGED || rbase + 1 < rows)) *reinterpret_cast<double2 *>(a.w + r0 + rbase) = make_double2(wn[0], wn[EU - 1]);
+        else {
+#pragma unroll
+            for (int e = 0; e < EU; ++e)
+                if (!RAGGED || rbase + e < rows) a.w[r0 + rbase + e] = wn[e];
+        }
+        if (HAS_DOT) consumer_bar(); // every row of w1buf is in place before the second sweep reads it
+        release_w(dep_bits(wn[0]));
+        if (KIND == PASS_UPD) return;
+    } else {
+    // ---- update: p = sum_c dec(V)[rows, c] * hs_c over this warp's columns (hs_s holds PRE * hs_c) ------
     double p[GV];
 #pragma unroll
     for (int i = 0; i < GV; ++i) p[i] = 0.0;
@@ -355,10 +501,11 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
     consumer_bar();
     release_w(dep_bits(ss)); // the tile of w was consumed by the stores of the new w and by the norms
     if (KIND == PASS_UPD) return;
+    }
 
     // ---- second sweep over the resident chunks: u_c += sum_rows dec(V)[r, c] * w_new[r] -----------------
     double wreg[GV];
-    load_w(c.w1buf, wreg);
+    load_w((upd_rowmap<FMT, F, KIND>() && (wslot & 1)) ? c.red : c.w1buf, wreg);
     Ring r2 = tile_start;
 #pragma unroll
     for (int st = 0; st < kMaxChunks / T::CPS; ++st) {
@@ -592,7 +739,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
     }
     const int nst = (k + T::STAGE_COLS - 1) / T::STAGE_COLS; // stages per row tile
     if (HAS_UPD && tid < kConsumers) {
-        if (tid < kMaxRangeCols) hs_s[tid] = (tid < k) ? hs_v * T::Fm::PRE : 0.0;
+        if (tid < kMaxRangeCols) hs_s[tid] = (tid < k) ? hs_v * (upd_rowmap<FMT, F, KIND>() ? 1.0 : T::Fm::PRE) : 0.0;
         consumer_bar();
     }
     if (threadIdx.x == 0) TR(2);
