@@ -34,7 +34,7 @@ FORMAT_BYTES = {"fp64": 8, "fp32": 4, "fp16": 2, "int32": 4, "int16": 2}
 METRIC = "arnoldi_iters_per_sec"
 UNIT = "iters/s"
 PROFILE_EVERY = 8       # CUDA-event brackets around the kernels of every 8th Arnoldi step of the timed region
-REF_ITERS = 100         # Arnoldi steps per format in one step of the reference arm / cpu_baseline
+REF_ITERS = 60          # Arnoldi steps per format in one step of the reference arm / cpu_baseline
 WORKLOADS = {"C2": {}, "C1": {}, "C5": {}, "C4": {}, "C2small": {"name": "C2", "grid": 32}}
 
 
