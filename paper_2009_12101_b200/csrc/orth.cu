@@ -12,18 +12,22 @@
 // dot, update); the fused middle pass makes that three, and consecutive passes walk the rows in
 // opposite directions so that the tail of one pass is still in the 126 MB L2 when the next begins.
 //
-// Mapping.  The n rows are cut into tiles of R rows, R*B = F KB per column segment (F = 1, 2, 4);
-// a tile is the sequence of column chunks [8 columns x R rows].  One persistent CTA per SM owns a
-// contiguous range of row tiles.  A producer warp streams chunks into a ring of shared-memory
-// stages (up to ~210 KB) with 1D bulk TMA copies (one copy per column segment, completion on an
-// mbarrier); sixteen consumer warps -- two row halves x eight columns -- work on a chunk as soon as
-// it lands: a warp owns one column of every chunk and one half of the rows, its lanes own 16-byte
+// Mapping.  The n rows are cut into tiles of R rows, R*B = F KB per column segment (F = 1, 2, 4: the
+// largest that leaves every CTA at least twelve tiles); a tile is the sequence of 32 KB stages
+// [32/F columns x F KB].  One persistent CTA per SM takes the tiles t = CTA, CTA + grid, ... (the
+// CTAs sweep a contiguous window of the basis together).  A producer warp streams stages into a
+// ring of shared memory (up to ~190 KB) with 2D tensor-map TMA boxes [8 columns x 1-2 KB]
+// (completion on an mbarrier) and the tile of w into a 4-slot ring, swizzled (wswz); it issues the
+// first stages BEFORE griddepcontrol.wait -- the basis is never written by the predecessor kernel.
+// Sixteen consumer warps -- two row halves x eight columns -- work on a stage as soon as it lands:
+// a warp owns one column of every 8-column chunk and one half of the rows, its lanes own 16-byte
 // payload words, so shared-memory reads are conflict free and every warp ends up with the CTA's
-// complete partial sums of ITS columns over its rows.  For the update each warp accumulates its
-// columns' contribution to its rows; the eight partial row vectors are added in a fixed order
-// through shared memory.  In PASS_UPD_DOT all chunks of a row tile stay resident until the new w
-// of that tile is known, then are swept a second time while the ring prefetches the next tile.
-// CTA partials go to global memory; the last CTA to finish adds them in a fixed order
+// complete partial sums of ITS columns over its rows.  The plain update uses the row-owner mapping
+// instead (each thread its own rows, all columns: no cross-warp reduction); the fused kind with
+// reduced storage accumulates per column-warp and adds the eight partial row vectors in a fixed
+// order through shared memory.  In PASS_UPD_DOT all stages of a row tile stay resident until the
+// new w of that tile is known, then are swept a second time while the ring prefetches the next
+// tile.  CTA partials go to global memory; the last CTA to finish adds them in a fixed order
 // (deterministic, no fp64 atomics), applies the per-vector scales and takes the decisions of
 // Fig. 1 lines 7 and 12 on the device.
 #include <cuda.h> // CUtensorMap (types only; the encoder is fetched with cudaGetDriverEntryPoint)
@@ -339,11 +343,7 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
     // chunks of stage `st` in which this warp's column exists
     auto valid_chunks = [&](int st) {
         const int left = c.k - st * T::STAGE_COLS - c.cw; // > 0 iff the column exists in chunk 0
-#ifdef CBG_PROBE_NV // development probe: cap the work per stage (0 = consumers only wait and release)
-        return left <= 0 ? 0 : min(min(T::CPS, CBG_PROBE_NV), (left + kChunkCols - 1) / kChunkCols);
-#else
         return left <= 0 ? 0 : min(T::CPS, (left + kChunkCols - 1) / kChunkCols);
-#endif
     };
     // Slots are handed back with mbar_arrive_after_use: `dep` carries a data dependency on everything
     // that was loaded from the slot (device_utils.cuh).
