@@ -297,15 +297,17 @@ def run_ours(args) -> int:
     d = fam[dom]
     achieved = d["bytes"] / (d["ms"] * 1e-3) / 1e9 if d["ms"] > 0 else 0.0
     # ncu dram__bytes_read + dram__bytes_write of this family, per launch: the ratio traffic / algorithmic
-    # bytes of the captured launches (profiles/ncu_traffic.json, written from the --set full captures)
+    # bytes of the captured launches (profiles/ncu_traffic.csv, written from the --set full captures)
     # applied to the average launch of this run
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     if os.path.exists(tpath):
-        with open(tpath) as f:
-            t = json.load(f).get(dom)
-        if t and d["launches"]:
-            traffic = round(t["traffic_over_algorithmic"] * d["bytes"] / d["launches"])
+        import csv
+
+        with open(tpath, newline="") as f:
+            ratios = {r["family"]: float(r["traffic_over_algorithmic"]) for r in csv.DictReader(f)}
+        if dom in ratios and d["launches"]:
+            traffic = round(ratios[dom] * d["bytes"] / d["launches"])
     roofline = {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
                 "frac": round(achieved / peak, 4), "traffic": traffic, "peak_source": peak_src,
                 "launches": d["launches"], "avg_launch_us": round(1e3 * d["ms"] / max(d["launches"], 1), 2),
