@@ -99,6 +99,12 @@ __device__ __forceinline__ void fence_proxy_async()
 {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
+// Barrier among the eight warps of one row half (ids 2 and 3): in the column-mapped update the two
+// halves of a tile never exchange data, so they need not wait for each other.
+__device__ __forceinline__ void half_bar(int half)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(2 + half), "n"(kConsumers / 2) : "memory");
+}
 __device__ __forceinline__ void consumer_bar()
 {
     asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory");
@@ -482,9 +488,9 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
 #pragma unroll
         for (int v = 0; v < VEC; v += 2)
             *reinterpret_cast<double2 *>(redw + wswz<VEC>(redw_s, (wi0 + f * 32) * VEC + v)) = make_double2(p[f * VEC + v], p[f * VEC + v + 1]);
-    consumer_bar();
-    // new w of the tile: the eight partial row vectors are added in a fixed order
-    for (int r = c.ct; r < R; r += kConsumers) {
+    half_bar(c.half);
+    // new w of this half's rows: the eight partial row vectors are added in a fixed order
+    for (int r = c.half * (R / 2) + (c.ct & (kConsumers / 2 - 1)); r < (c.half + 1) * (R / 2); r += kConsumers / 2) {
         double tot = 0.0;
 #pragma unroll
         for (int q = 0; q < kColWarps; ++q) tot += c.red[q * R + wswz<VEC>(red_s + q * R * 8, r)]; // stored like the w tiles: conflict-free both ways
@@ -498,7 +504,7 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
         }
         if (HAS_DOT) c.w1buf[wswz<VEC>(w1_s, r)] = live ? wn : 0.0; // kept apart from the TMA-written slot: no proxy fence
     }
-    consumer_bar();
+    half_bar(c.half);
     release_w(dep_bits(ss)); // the tile of w was consumed by the stores of the new w and by the norms
     if (KIND == PASS_UPD) return;
     }
@@ -799,6 +805,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
         if (HAS_UPD) {
             ss = warp_sum(ss);
             am = warp_max(am);
+            consumer_bar(); // the other row half may still be adding the partial row vectors of its last tile out of `red`
             if (lane == 0) {
                 red[warp] = ss;
                 red[kConsumerWarps + warp] = am;
