@@ -832,6 +832,164 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
     if (threadIdx.x == 0) TR(23);
 }
 
+
+// ---- few vectors (k <= 8): no staging --------------------------------------------------------------------
+// With at most eight basis vectors a row tile is a few KB and the staged kernel is bound by its
+// per-tile round trips (multi-dot, n = 4.2e6: 50 us for k = 1..4, whatever the format).  Here a thread
+// takes one 16-byte payload word of every vector plus the matching rows of w straight from global
+// memory -- all loads of an iteration in flight together -- keeps the k words in registers for
+// both sweeps of the fused kind, and the CTA reduces its partial sums through shuffles; the
+// last-block-done final stage is the same as in orth_kernel.
+constexpr int kSmallK = 8;
+
+template <int FMT> __device__ __forceinline__ void decode_true(const uint4 &r, double (&d)[Fmt<FMT>::VEC])
+{
+    if constexpr (FMT == CBGMRES_FP64) {
+        d[0] = __hiloint2double((int)r.y, (int)r.x);
+        d[1] = __hiloint2double((int)r.w, (int)r.z);
+    } else if constexpr (FMT == CBGMRES_FP32) {
+        d[0] = (double)__uint_as_float(r.x);
+        d[1] = (double)__uint_as_float(r.y);
+        d[2] = (double)__uint_as_float(r.z);
+        d[3] = (double)__uint_as_float(r.w);
+    } else if constexpr (FMT == CBGMRES_INT32) {
+        d[0] = (double)(int)r.x;
+        d[1] = (double)(int)r.y;
+        d[2] = (double)(int)r.z;
+        d[3] = (double)(int)r.w;
+    } else if constexpr (FMT == CBGMRES_FP16) {
+        half2_cvt(r.x, d[0], d[1]);
+        half2_cvt(r.y, d[2], d[3]);
+        half2_cvt(r.z, d[4], d[5]);
+        half2_cvt(r.w, d[6], d[7]);
+    } else {
+        i16x2_cvt(r.x, d[0], d[1]);
+        i16x2_cvt(r.y, d[2], d[3]);
+        i16x2_cvt(r.z, d[4], d[5]);
+        i16x2_cvt(r.w, d[6], d[7]);
+    }
+}
+
+template <int FMT, int KIND> __global__ void __launch_bounds__(kOrthThreads, 1) orth_small_kernel(const OrthArgs a)
+{
+    using Fm = Fmt<FMT>;
+    constexpr int VEC = Fm::VEC, B = Fm::BYTES, NW = kOrthThreads / 32;
+    constexpr bool HAS_UPD = KIND != PASS_DOT, HAS_DOT = KIND != PASS_UPD;
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ double s_part[NW][kSmallK], s_nrm[2 * NW];
+    Ctl *ctl = a.ctl;
+    pdl_wait();
+    pdl_launch_dependents();
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, k = a.k;
+    const int stop_after = __ldcg(&ctl->stop_after), reorth_flag = __ldcg(&ctl->reorth_flag);
+    double coef[kSmallK];
+#pragma unroll
+    for (int c = 0; c < kSmallK; ++c) coef[c] = (HAS_UPD && c < k) ? __ldcg(&a.hs[c]) : 0.0;
+    if (a.mode == MODE_ORTH1 || a.mode == MODE_ORTH2) {
+        if (a.step > stop_after) return;
+        if (a.mode == MODE_ORTH2 && !reorth_flag) return;
+    }
+    double acc[kSmallK];
+#pragma unroll
+    for (int c = 0; c < kSmallK; ++c) acc[c] = 0.0;
+    double ss = 0.0, am = 0.0;
+    const unsigned char *V = static_cast<const unsigned char *>(a.V);
+    const int64_t colb = a.ld * B, ngroups = a.n / VEC;
+    for (int64_t g = (int64_t)blockIdx.x * kOrthThreads + tid; g < ngroups; g += (int64_t)gridDim.x * kOrthThreads) {
+        uint4 raw[kSmallK];
+#pragma unroll
+        for (int c = 0; c < kSmallK; ++c)
+            if (c < k) raw[c] = __ldg(reinterpret_cast<const uint4 *>(V + c * colb + g * 16));
+        double wv[VEC];
+#pragma unroll
+        for (int v = 0; v < VEC; v += 2) {
+            const double2 t = *reinterpret_cast<const double2 *>(a.w + g * VEC + v);
+            wv[v] = t.x;
+            wv[v + 1] = t.y;
+        }
+        if (HAS_UPD) {
+            double p[VEC];
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) p[v] = 0.0;
+#pragma unroll
+            for (int c = 0; c < kSmallK; ++c)
+                if (c < k) {
+                    double d[VEC];
+                    decode_true<FMT>(raw[c], d);
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) p[v] = fma(d[v], coef[c], p[v]);
+                }
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                wv[v] -= p[v];
+                ss = fma(wv[v], wv[v], ss);
+                am = fmax(am, fabs(wv[v]));
+            }
+#pragma unroll
+            for (int v = 0; v < VEC; v += 2) *reinterpret_cast<double2 *>(a.w + g * VEC + v) = make_double2(wv[v], wv[v + 1]);
+        }
+        if (HAS_DOT) {
+#pragma unroll
+            for (int c = 0; c < kSmallK; ++c)
+                if (c < k) {
+                    double d[VEC];
+                    decode_true<FMT>(raw[c], d);
+                    acc[c] += word_dot<VEC>(d, wv);
+                }
+        }
+    }
+    if (blockIdx.x == 0 && tid == 0) { // the last n mod VEC rows, one by one
+        for (int64_t r = ngroups * VEC; r < a.n; ++r) {
+            double wr = a.w[r];
+            if (HAS_UPD) {
+                double p = 0.0;
+                for (int c = 0; c < k; ++c) p = fma(Fm::decode_one(V + c * colb, r), coef[c], p);
+                wr -= p;
+                a.w[r] = wr;
+                ss = fma(wr, wr, ss);
+                am = fmax(am, fabs(wr));
+            }
+            if (HAS_DOT)
+                for (int c = 0; c < k; ++c) acc[c] = fma(Fm::decode_one(V + c * colb, r), wr, acc[c]);
+        }
+    }
+    // ---- CTA partials: shuffles inside the warps, then the warps in a fixed order --------------------------
+    if (HAS_DOT) {
+#pragma unroll
+        for (int c = 0; c < kSmallK; ++c) {
+            const double t = warp_sum(acc[c]);
+            if (lane == 0) s_part[warp][c] = t;
+        }
+    }
+    if (HAS_UPD) {
+        ss = warp_sum(ss);
+        am = warp_max(am);
+        if (lane == 0) {
+            s_nrm[warp] = ss;
+            s_nrm[NW + warp] = am;
+        }
+    }
+    __syncthreads();
+    if (HAS_DOT && tid < k) {
+        double t = 0.0;
+#pragma unroll
+        for (int q = 0; q < NW; ++q) t += s_part[q][tid];
+        a.partials[(size_t)blockIdx.x * kLdp + tid] = t;
+    }
+    if (HAS_UPD && tid == 0) {
+        double t = 0.0, m = 0.0;
+#pragma unroll
+        for (int q = 0; q < NW; ++q) {
+            t += s_nrm[q];
+            m = fmax(m, s_nrm[NW + q]);
+        }
+        a.npart[blockIdx.x] = t;
+        a.npart[kMaxGrid + blockIdx.x] = m;
+    }
+    if (!last_block_done(&ctl->tickets[0])) return;
+    orth_finalize<KIND, Fm::SCALED>(a, k, reinterpret_cast<double *>(smem));
+}
+
 // ---- launchers ---------------------------------------------------------------------------------------
 namespace {
 
@@ -997,6 +1155,32 @@ template <int FMT, int F, int KIND> int launch_inst(cudaStream_t s, OrthArgs &a)
     return 1;
 }
 
+constexpr int kSmallSmemBytes = 17 * 1024; // the final stage's scratch ([16][128] doubles)
+
+template <int KIND> int launch_small(cudaStream_t s, int format, OrthArgs &a)
+{
+    const int64_t groups = a.n / (16 / fmt_bytes(format));
+    int64_t grid = (groups + kOrthThreads - 1) / kOrthThreads;
+    if (grid > kNumSMs) grid = kNumSMs;
+    if (grid < 1) grid = 1;
+    const dim3 g((unsigned)grid), b(kOrthThreads);
+    switch (format) {
+    case CBGMRES_FP64: launch_chain(orth_small_kernel<CBGMRES_FP64, KIND>, g, b, kSmallSmemBytes, s, a); break;
+    case CBGMRES_FP32: launch_chain(orth_small_kernel<CBGMRES_FP32, KIND>, g, b, kSmallSmemBytes, s, a); break;
+    case CBGMRES_FP16: launch_chain(orth_small_kernel<CBGMRES_FP16, KIND>, g, b, kSmallSmemBytes, s, a); break;
+    case CBGMRES_INT32: launch_chain(orth_small_kernel<CBGMRES_INT32, KIND>, g, b, kSmallSmemBytes, s, a); break;
+    case CBGMRES_INT16: launch_chain(orth_small_kernel<CBGMRES_INT16, KIND>, g, b, kSmallSmemBytes, s, a); break;
+    default: return 0;
+    }
+    return 1;
+}
+// k <= 8, column count known on the host, segment size not pinned by the caller, 16-byte aligned columns
+inline bool use_small(const OrthArgs &a, int format, int forced_seg_kb)
+{
+    return a.k <= kSmallK && !a.d_k && forced_seg_kb == 0 && (a.ld * fmt_bytes(format)) % 16 == 0 &&
+           reinterpret_cast<uintptr_t>(a.V) % 16 == 0 && reinterpret_cast<uintptr_t>(a.w) % 16 == 0;
+}
+
 template <int FMT, int KIND> int launch_f(cudaStream_t s, OrthArgs &a, int seg_kb)
 {
     constexpr int VEC = Fmt<FMT>::VEC;
@@ -1076,7 +1260,8 @@ int launch_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b, int64
         a.h_out = h_out + c0;
         a.hs_out = hs_out ? hs_out + c0 : nullptr;
         a.last_range = (c0 + kMaxRangeCols >= k);
-        launches += launch_fmt<PASS_DOT>(s, b.format, a, choose_seg_kb(b.format, PASS_DOT, kk, n, seg_kb));
+        if (use_small(a, b.format, seg_kb)) launches += launch_small<PASS_DOT>(s, b.format, a);
+        else launches += launch_fmt<PASS_DOT>(s, b.format, a, choose_seg_kb(b.format, PASS_DOT, kk, n, seg_kb));
     }
     return launches;
 }
@@ -1098,7 +1283,8 @@ int launch_update(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t
         a.w = w;
         a.k = kk;
         a.last_range = (c0 + kMaxRangeCols >= k);
-        launches += launch_fmt<PASS_UPD>(s, b.format, a, choose_seg_kb(b.format, PASS_UPD, kk, n, seg_kb));
+        if (use_small(a, b.format, seg_kb)) launches += launch_small<PASS_UPD>(s, b.format, a);
+        else launches += launch_fmt<PASS_UPD>(s, b.format, a, choose_seg_kb(b.format, PASS_UPD, kk, n, seg_kb));
     }
     return launches;
 }
@@ -1119,6 +1305,7 @@ int launch_update_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b
     a.k = k;
     a.h_out = h_out;
     a.hs_out = hs_out;
+    if (use_small(a, b.format, seg_kb)) return launch_small<PASS_UPD_DOT>(s, b.format, a);
     return launch_fmt<PASS_UPD_DOT>(s, b.format, a, choose_seg_kb(b.format, PASS_UPD_DOT, k, n, seg_kb));
 }
 
