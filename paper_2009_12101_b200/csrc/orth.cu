@@ -557,6 +557,9 @@ template <int KIND, bool SCALED> __device__ void orth_finalize(const OrthArgs &a
     const int nsl = 512 / kc, col = tid & (kc - 1), sl = tid / kc;
     const int per = (nb + nsl - 1) / nsl;
     double *part = scratch; // [nsl][kMaxRangeCols]
+    // sigma_c of the column this thread finishes below: fetched with the partials, not after them
+    double sigma_v = 1.0;
+    if (HAS_DOT && SCALED && tid < k) sigma_v = __ldcg(&a.scales[tid]);
     if (HAS_DOT && tid < 512) {
         double sum = 0.0;
         if (col < k) {
@@ -570,6 +573,7 @@ template <int KIND, bool SCALED> __device__ void orth_finalize(const OrthArgs &a
             }
         }
         part[sl * kMaxRangeCols + col] = sum;
+        if (tid == 0) TR(24);
     }
     if (HAS_UPD && a.last_range) {
         nt = warp_sum(nt);
@@ -580,6 +584,7 @@ template <int KIND, bool SCALED> __device__ void orth_finalize(const OrthArgs &a
         }
     }
     __syncthreads();
+    if (tid == 0) TR(25);
     if (HAS_UPD && a.last_range && tid == 0) {
         double t = 0.0, m = 0.0;
 #pragma unroll
@@ -615,10 +620,10 @@ template <int KIND, bool SCALED> __device__ void orth_finalize(const OrthArgs &a
     if (HAS_UPD && HAS_DOT) __syncthreads(); // s_apply
     if (HAS_DOT) {
         const bool apply = s_apply != 0;
-        for (int c = tid; c < k; c += kOrthThreads) {
+        for (int c = tid; c < k; c += kOrthThreads) { // k <= kMaxRangeCols < kOrthThreads: c == tid
             double tot = 0.0;
             for (int q = 0; q < nsl; ++q) tot += part[q * kMaxRangeCols + c];
-            const double sigma = SCALED ? a.scales[c] : 1.0;
+            const double sigma = sigma_v;
             const double h = tot * sigma; // h_c = sigma_c * sum_i q_ic w_i
             if (KIND == PASS_DOT) {
                 if (a.mode == MODE_ORTH2) a.h_out[c] += h; // Fig. 1 l.9: h_{1:j,j} += u
