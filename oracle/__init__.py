@@ -68,6 +68,12 @@ def lib():
                                 C.POINTER(_Params), C.POINTER(_Result), C.c_void_p, C.c_int32, C.c_void_p, C.c_int32,
                                 C.POINTER(_Capture)]
         L.orc_gmres.restype = C.c_int
+        L.orc_gmres_m.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                  C.POINTER(_Params), C.POINTER(_Result), C.c_void_p, C.c_int32, C.c_void_p, C.c_int32,
+                                  C.POINTER(_Capture)]
+        L.orc_gmres_m.restype = C.c_int
+        L.orc_jacobi_diag.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_jacobi_diag.restype = None
         _lib = L
     return _lib
 
@@ -186,9 +192,19 @@ class OracleResult:
     capture: dict = field(default_factory=dict)
 
 
+def jacobi_diag(A) -> np.ndarray:
+    """M = diag(A) of the scalar Jacobi preconditioner; absent / zero entries give 1."""
+    d = np.empty(A.n)
+    lib().orc_jacobi_diag(A.n, _p(A.row_ptr), _p(A.col_idx), _p(A.vals), _p(d))
+    return d
+
+
 def gmres(A, b, x0, restart: int, rel_tol: float, max_iters: int, fmt: str = "fp64", reorth: str = "cond",
-          eta: float = 1.0 / math.sqrt(2.0), capture_cycle: int | None = None) -> OracleResult:
-    """Restarted CB-GMRES (Fig. 1).  See orc_gmres in cbgmres_oracle.c."""
+          eta: float = 1.0 / math.sqrt(2.0), capture_cycle: int | None = None, precond: str = "none") -> OracleResult:
+    """Restarted CB-GMRES (Fig. 1).  See orc_gmres_m in cbgmres_oracle.c.
+    precond = "jacobi": right preconditioner M = diag(A) (Fig. 1 l.3 and l.17)."""
+    if precond not in ("none", "jacobi"):
+        raise ValueError(precond)
     b = _f64(b)
     x = _f64(x0).copy()
     n, m = A.n, restart
@@ -202,8 +218,10 @@ def gmres(A, b, x0, restart: int, rel_tol: float, max_iters: int, fmt: str = "fp
         bufs = dict(Vhat=np.zeros((m + 1, n)), Vfp64=np.zeros((m + 1, n)), Hbar=np.zeros((m, m + 1)),
                     y=np.zeros(m), g=np.zeros(m + 1))
         cap = _Capture(capture_cycle, 0, 0.0, *[bufs[k].ctypes.data for k in ("Vhat", "Vfp64", "Hbar", "y", "g")])
-    rc = lib().orc_gmres(n, _p(A.row_ptr), _p(A.col_idx), _p(A.vals), _p(b), _p(x), C.byref(prm), C.byref(res),
-                         _p(rec), rec.shape[0], _p(expl), expl.shape[0], C.byref(cap) if cap else None)
+    mdiag = jacobi_diag(A) if precond == "jacobi" else None
+    rc = lib().orc_gmres_m(n, _p(A.row_ptr), _p(A.col_idx), _p(A.vals), _p(mdiag) if mdiag is not None else None,
+                           _p(b), _p(x), C.byref(prm), C.byref(res), _p(rec), rec.shape[0], _p(expl), expl.shape[0],
+                           C.byref(cap) if cap else None)
     if rc != 0:
         raise RuntimeError(f"orc_gmres failed with {rc}")
     capture = {}

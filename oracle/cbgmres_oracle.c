@@ -380,9 +380,35 @@ typedef struct {      /* optional capture of one restart cycle, for the pins */
     double *g;        /* out: m+1, rotated right-hand side at the end of the cycle */
 } orc_capture;
 
+/* Scalar Jacobi preconditioner M = diag(A) ("a scalar Jacobi preconditioner" in every
+ * experiment): d_i = a_ii; a missing or zero diagonal entry leaves that row unscaled (d_i = 1). */
+void orc_jacobi_diag(int64_t n, const int32_t *rp, const int32_t *ci, const double *va, double *d)
+{
+    for (int64_t i = 0; i < n; i++) {
+        d[i] = 1.0;
+        for (int32_t p = rp[i]; p < rp[i + 1]; p++)
+            if (ci[p] == i && va[p] != 0.0) d[i] = va[p];
+    }
+}
+
+/* Fig. 1 with a right preconditioner M = diag(mdiag) (mdiag == NULL: M = I):
+ * l.3 "w := A (M^-1 v_j)" and l.17 "x_m := x_0 + M^-1 (V_m y_m)"; the residual
+ * of l.1 and the stopping test are those of the ORIGINAL system A x = b (right preconditioning
+ * leaves the residual unchanged). */
+int orc_gmres_m(int64_t n, const int32_t *rp, const int32_t *ci, const double *va, const double *mdiag,
+                const double *b, double *x, const orc_params *prm, orc_result *res, double *rec_hist,
+                int32_t rec_hist_cap, double *expl_hist, int32_t expl_hist_cap, orc_capture *cap);
+
 int orc_gmres(int64_t n, const int32_t *rp, const int32_t *ci, const double *va, const double *b, double *x,
               const orc_params *prm, orc_result *res, double *rec_hist, int32_t rec_hist_cap, double *expl_hist,
               int32_t expl_hist_cap, orc_capture *cap)
+{
+    return orc_gmres_m(n, rp, ci, va, NULL, b, x, prm, res, rec_hist, rec_hist_cap, expl_hist, expl_hist_cap, cap);
+}
+
+int orc_gmres_m(int64_t n, const int32_t *rp, const int32_t *ci, const double *va, const double *mdiag,
+                const double *b, double *x, const orc_params *prm, orc_result *res, double *rec_hist,
+                int32_t rec_hist_cap, double *expl_hist, int32_t expl_hist_cap, orc_capture *cap)
 {
     const int m = prm->restart, fmt = prm->format;
     const int64_t B = orc_format_bytes(fmt);
@@ -394,11 +420,12 @@ int orc_gmres(int64_t n, const int32_t *rp, const int32_t *ci, const double *va,
     double *v = (double *)malloc((size_t)n * 8);   /* fp64 copy of the newest basis vector (reading Q1) */
     double *w = (double *)malloc((size_t)n * 8);
     double *tmp = (double *)malloc((size_t)n * 8); /* one decoded basis vector */
+    double *z = (double *)malloc((size_t)n * 8);   /* M^-1 v (l.3) / V_k y (l.17) when preconditioned */
     double *h = (double *)calloc((size_t)m + 2, 8), *u = (double *)calloc((size_t)m + 2, 8);
     double *R = (double *)calloc((size_t)(m + 1) * (size_t)m, 8); /* rotated H, column-major ld m+1 */
     double *cs = (double *)calloc((size_t)m, 8), *sn = (double *)calloc((size_t)m, 8);
     double *g = (double *)calloc((size_t)m + 1, 8), *y = (double *)calloc((size_t)m, 8);
-    if (!V || !sigma || !v || !w || !tmp || !h || !u || !R || !cs || !sn || !g || !y) return 2;
+    if (!V || !sigma || !v || !w || !tmp || !z || !h || !u || !R || !cs || !sn || !g || !y) return 2;
 #define VCOL(c) (V + (size_t)(c) * (size_t)n * (size_t)B)
 
     memset(res, 0, sizeof(*res));
@@ -439,8 +466,14 @@ int orc_gmres(int64_t n, const int32_t *rp, const int32_t *ci, const double *va,
         }
         int k = 0, breakdown = 0;
         for (int j = 1; j <= m; j++) {
-            /* l.3: w := A v   (the fp64 v, reading Q1; M = I) */
-            orc_spmv(n, rp, ci, va, v, w);
+            /* l.3: w := A (M^-1 v)   (the fp64 v, reading Q1) */
+            if (mdiag) {
+#pragma omp parallel for schedule(static)
+                for (i = 0; i < n; i++) z[i] = v[i] / mdiag[i];
+                orc_spmv(n, rp, ci, va, z, w);
+            } else {
+                orc_spmv(n, rp, ci, va, v, w);
+            }
             /* l.4: omega := ||w||_2 */
             const double omega = nrm2(n, w);
             /* l.5: h_{1:j,j} := V_j^T w  (classical Gram-Schmidt: all j dots from the same w) */
@@ -519,10 +552,20 @@ int orc_gmres(int64_t n, const int32_t *rp, const int32_t *ci, const double *va,
             for (int c = r + 1; c < k; c++) s -= R[(size_t)c * (m + 1) + r] * y[c];
             y[r] = s / R[(size_t)r * (m + 1) + r];
         }
-        /*       x := x_0 + V_k y   (decoded basis) */
-        for (int c = 0; c < k; c++) {
-            orc_dec(fmt, n, VCOL(c), sigma[c], tmp);
-            axpy(n, y[c], tmp, x);
+        /*       x := x_0 + M^-1 (V_k y)   (decoded basis) */
+        if (mdiag) {
+            memset(z, 0, (size_t)n * 8);
+            for (int c = 0; c < k; c++) {
+                orc_dec(fmt, n, VCOL(c), sigma[c], tmp);
+                axpy(n, y[c], tmp, z);
+            }
+#pragma omp parallel for schedule(static)
+            for (i = 0; i < n; i++) x[i] += z[i] / mdiag[i];
+        } else {
+            for (int c = 0; c < k; c++) {
+                orc_dec(fmt, n, VCOL(c), sigma[c], tmp);
+                axpy(n, y[c], tmp, x);
+            }
         }
         if (capture) {
             cap->k = k;
@@ -535,6 +578,6 @@ done:
     res->iters = iters;
     res->restarts = cycles;
 #undef VCOL
-    free(V); free(sigma); free(v); free(w); free(tmp); free(h); free(u); free(R); free(cs); free(sn); free(g); free(y);
+    free(V); free(sigma); free(v); free(w); free(tmp); free(z); free(h); free(u); free(R); free(cs); free(sn); free(g); free(y);
     return 0;
 }

@@ -202,3 +202,100 @@ def test_breakdown_on_invariant_subspace():
     r = oracle.gmres(A, b, np.zeros(n), restart=5, rel_tol=1e-12, max_iters=20)
     assert r.converged and r.iters == 1 and r.breakdown == 1
     assert np.allclose(r.x, b / 3.0, rtol=1e-15)
+
+
+# ---- scalar Jacobi right preconditioner (Fig. 1 l.3 "w := A(M^-1 v_j)", l.17 "x_0 + M^-1(V_m y_m)") ----
+
+def _badly_scaled_system(n, seed):
+    """Dense nonsymmetric system whose diagonal spans four orders of magnitude (column scaling of a
+    well-conditioned matrix): input construction only."""
+    from workloads import CSR
+    import scipy.sparse as sp
+
+    _, Ad, b = random_dense_system(n, seed)
+    col = 10.0 ** np.random.default_rng(seed + 1).uniform(-2.0, 2.0, n)
+    col[::3] *= -1.0  # negative diagonal entries too: M^-1 is a division by d_i, not by |d_i|
+    Ad = Ad * col[None, :]
+    S = sp.csr_matrix(Ad)
+    S.sort_indices()
+    return CSR(n, S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(np.float64)), Ad, b
+
+
+def test_jacobi_diag_is_the_matrix_diagonal():
+    A, Ad, _ = _badly_scaled_system(17, 70)
+    assert np.array_equal(oracle.jacobi_diag(A), np.diag(Ad))
+    p = make_config("C1", grid=6)
+    assert np.array_equal(oracle.jacobi_diag(p.A), np.full(p.A.n, 4.0))
+    # a row without a stored diagonal entry is left unscaled
+    from workloads import CSR
+    B = CSR(2, np.array([0, 1, 2], np.int32), np.array([1, 1], np.int32), np.array([5.0, 7.0]))
+    assert np.array_equal(oracle.jacobi_diag(B), np.array([1.0, 7.0]))
+
+
+@pytest.mark.parametrize("n,seed", [(12, 71), (40, 72)])
+def test_jacobi_tiny_dense_matches_direct_solve(n, seed):
+    A, Ad, b = _badly_scaled_system(n, seed)
+    x0 = np.random.default_rng(seed + 2).standard_normal(n)
+    r = oracle.gmres(A, b, x0, restart=n, rel_tol=1e-13, max_iters=4 * n, fmt="fp64", precond="jacobi")
+    xs = np.linalg.solve(Ad, b)
+    assert r.converged and r.iters <= n + 1
+    assert np.linalg.norm(r.x - xs) <= 1e-9 * np.linalg.norm(xs)
+    # the stopping test is on the residual of the ORIGINAL system
+    assert np.linalg.norm(b - Ad @ r.x) <= 1e-13 * np.linalg.norm(b) * (1 + 1e-6)
+
+
+def test_jacobi_equals_plain_gmres_on_the_column_scaled_matrix():
+    """Right preconditioning is GMRES on A M^-1 in the variable u = M x with the SAME residuals:
+    the recurrence history of the preconditioned run on A equals that of the plain run on the
+    explicitly formed A D^-1 (scipy, input construction), and x = D^-1 u.  A left-preconditioned or
+    un-preconditioned implementation, or one that drops M^-1 in l.17, fails here."""
+    from workloads import CSR
+    import scipy.sparse as sp
+
+    n = 60
+    A, Ad, b = _badly_scaled_system(n, 73)
+    d = np.diag(Ad).copy()
+    S = sp.csr_matrix(Ad / d[None, :])
+    S.sort_indices()
+    Ahat = CSR(n, S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(np.float64))
+    kw = dict(restart=3, rel_tol=1e-11, max_iters=400, fmt="fp64")
+    rp = oracle.gmres(A, b, np.zeros(n), precond="jacobi", **kw)
+    ru = oracle.gmres(Ahat, b, np.zeros(n), precond="none", **kw)
+    assert rp.converged and ru.converged and rp.restarts > 2
+    assert rp.iters == ru.iters
+    live = ru.rec_history > 1e-9
+    assert np.allclose(rp.rec_history[live], ru.rec_history[live], rtol=1e-6)
+    assert np.linalg.norm(rp.x - ru.x / d) <= 1e-9 * np.linalg.norm(rp.x)
+    # and it is not the un-preconditioned iteration (which needs many more steps on this matrix)
+    r0 = oracle.gmres(A, b, np.zeros(n), precond="none", **kw)
+    assert (not r0.converged) or r0.iters > rp.iters
+
+
+@pytest.mark.parametrize("fmt", ["fp64", "fp32", "int16"])
+def test_jacobi_is_a_no_op_up_to_rounding_on_a_constant_diagonal(fmt):
+    """C2 has the constant diagonal 6: A D^-1 = A / 6 spans the same Krylov spaces, so the residual
+    history is that of the plain solver (the paper's stencil-like problems)."""
+    p = make_config("C2", grid=10)
+    kw = dict(restart=20, rel_tol=1e-8, max_iters=400, fmt=fmt)
+    a = oracle.gmres(p.A, p.b, p.x0, precond="none", **kw)
+    j = oracle.gmres(p.A, p.b, p.x0, precond="jacobi", **kw)
+    assert a.converged and j.converged
+    assert abs(a.iters - j.iters) <= (0 if fmt == "fp64" else 2)
+    if fmt == "fp64":
+        live = a.rec_history > 1e-7
+        assert np.allclose(a.rec_history[live], j.rec_history[live], rtol=1e-6)
+    S = p.A.to_scipy()
+    assert np.linalg.norm(p.b - S @ j.x) <= 1e-8 * np.linalg.norm(p.b)
+
+
+def test_jacobi_makes_the_power_law_config_converge():
+    """C4's diagonal (1.1 x row abs-sum of power-law rows) spans orders of magnitude; with the paper's
+    default preconditioner the restarted solver converges where M = I stalls."""
+    p = make_config("C4", n=3000)
+    kw = dict(restart=p.restart, rel_tol=p.rel_tol, max_iters=600, fmt="fp64")
+    j = oracle.gmres(p.A, p.b, p.x0, precond="jacobi", **kw)
+    assert j.converged
+    S = p.A.to_scipy()
+    assert np.linalg.norm(p.b - S @ j.x) <= p.rel_tol * np.linalg.norm(p.b) * (1 + 1e-6)
+    a = oracle.gmres(p.A, p.b, p.x0, precond="none", **kw)
+    assert (not a.converged) or a.iters > 2 * j.iters
