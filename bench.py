@@ -35,6 +35,7 @@ METRIC = "arnoldi_iters_per_sec"
 UNIT = "iters/s"
 PROFILE_EVERY = 8       # CUDA-event brackets around the kernels of every 8th Arnoldi step of the timed region
 REF_ITERS = 60          # Arnoldi steps per format in one step of the reference arm / cpu_baseline
+PRECOND = "none"        # --precond jacobi: the paper's scalar Jacobi right preconditioner on both arms
 WORKLOADS = {"C2": {}, "C1": {}, "C5": {}, "C4": {}, "C2small": {"name": "C2", "grid": 32}}
 
 
@@ -122,7 +123,7 @@ def _oracle_step(p, iters_per_format: int):
     t0 = time.perf_counter()
     done = 0
     for fmt in p.formats:
-        r = oracle.gmres(p.A, p.b, p.x0, p.restart, p.rel_tol, iters_per_format, fmt)
+        r = oracle.gmres(p.A, p.b, p.x0, p.restart, p.rel_tol, iters_per_format, fmt, precond=PRECOND)
         done += r.iters
     return done, time.perf_counter() - t0
 
@@ -153,7 +154,7 @@ def run_reference(args) -> int:
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * total_s / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "n": p.A.n, "nnz": p.A.nnz, "restart": p.restart, "rel_tol": p.rel_tol,
+        "config": {"workload": args.workload, "precond": PRECOND, "n": p.A.n, "nnz": p.A.nnz, "restart": p.restart, "rel_tol": p.rel_tol,
                    "formats": list(p.formats), "bounded_sample": _sample_text(p, REF)},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": _sample_text(p, REF)},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -170,12 +171,12 @@ def _solve_all_formats(solver, p, dev, host=None):
     for fmt in p.formats:
         if host is None:
             solver.profile_reset()
-            _, r = solver.solve(dev["b"], dev["x0"], p.restart, p.rel_tol, p.max_iters, fmt)
+            _, r = solver.solve(dev["b"], dev["x0"], p.restart, p.rel_tol, p.max_iters, fmt, precond=PRECOND)
             r.prof = solver.profile_get()
         else:
             host["x"].copy_(host["x0"])
             r = solver.solve_host(host["row_ptr"], host["col_idx"], host["vals"], host["b"], host["x"], p.restart,
-                                  p.rel_tol, p.max_iters, fmt)
+                                  p.rel_tol, p.max_iters, fmt, precond=PRECOND)
         out[fmt] = r
     return out
 
@@ -328,7 +329,7 @@ def run_ours(args) -> int:
         "metric": METRIC, "value": iters / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "n": n, "nnz": nnz, "restart": p.restart, "rel_tol": p.rel_tol,
+        "config": {"workload": args.workload, "precond": PRECOND, "n": n, "nnz": nnz, "restart": p.restart, "rel_tol": p.rel_tol,
                    "max_iters": p.max_iters, "formats": list(p.formats), "reorth": "cond (eta = 1/sqrt 2)",
                    "step": "one solve to convergence per storage format",
                    "l2": "no flush: basis (0.2-0.8 GB) + matrix exceed the 126 MB L2; reuse inside a solve is the workload's own",
@@ -354,7 +355,10 @@ def main() -> int:
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
     ap.add_argument("--workload", choices=tuple(WORKLOADS), default="C2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--precond", choices=("none", "jacobi"), default="none")
     args = ap.parse_args()
+    global PRECOND
+    PRECOND = args.precond
     if args.steps < 1:
         ap.error("--steps must be >= 1")
     if args.impl == "reference":

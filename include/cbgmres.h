@@ -65,6 +65,12 @@ typedef enum {
     CBGMRES_NOT_CONVERGED = 16 /* ran to max_iters; x is valid, result is filled */
 } cbgmres_status_t;
 
+/* Right preconditioner M (Fig. 1 l.3 "w := A(M^-1 v_j)", l.17 "x_m := x_0 + M^-1(V_m y_m)").
+ * JACOBI: M = diag(A), the setting of every experiment in the paper; a row without a
+ * nonzero diagonal entry is left unscaled.  It costs one pass over the matrix per solve and nvals*8 +
+ * n*8 more workspace bytes (cbgmres_workspace_bytes accounts for them); the Arnoldi loop is unchanged. */
+typedef enum { CBGMRES_PRECOND_NONE = 0, CBGMRES_PRECOND_JACOBI = 1 } cbgmres_precond_t;
+
 #define CBGMRES_MAX_RESTART 512
 
 typedef struct {
@@ -76,7 +82,7 @@ typedef struct {
     double eta;              /* re-orthogonalisation threshold; 0 -> 1/sqrt(2) (reading Q3) */
     double *h_res_history;   /* optional HOST buffer: recurrence residual |g_{j+1}|/||b|| per Arnoldi step */
     int32_t res_history_cap; /* entries available in h_res_history (0 if unused) */
-    int32_t reserved;
+    int32_t precond;         /* cbgmres_precond_t: right preconditioner M of Fig. 1 l.3 / l.17 (0 = none) */
 } cbgmres_params;
 
 typedef struct {

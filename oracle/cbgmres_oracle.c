@@ -18,6 +18,8 @@
  *   - GMRES (fp64 storage): numpy.linalg.solve on tiny systems, <= n-step convergence, Arnoldi
  *     relation, basis orthogonality, recurrence == explicit residual, scipy.sparse.linalg.gmres;
  *   - GMRES (compressed storage): mixed Arnoldi relation, |V^| <= 1, explicit residual <= tol.
+ *   - right preconditioner M = diag(A) (orc_gmres_m): numpy.linalg.solve on badly scaled systems,
+ *     residual history equal to plain GMRES on the explicitly formed A D^-1, constant-diagonal no-op.
  *   - PARITY UNPINNED: exact iteration counts of the compressed formats on the synthetic configs
  *     (the paper prints no value for any of them; only Table 2's qualitative ratios apply).
  *

@@ -20,6 +20,7 @@ FORMATS = ("fp64", "fp32", "fp16", "int32", "int16")
 FORMAT_CODE = {f: i for i, f in enumerate(FORMATS)}
 FORMAT_BYTES = {"fp64": 8, "fp32": 4, "fp16": 2, "int32": 4, "int16": 2}
 REORTH_CODE = {"never": 0, "cond": 1, "always": 2}
+PRECOND_CODE = {"none": 0, "jacobi": 1}
 STATUS = {0: "OK", 1: "E_INVALID", 2: "E_NOMATRIX", 3: "E_WORKSPACE", 4: "E_CUDA", 5: "E_NONFINITE",
           16: "NOT_CONVERGED"}
 MAX_RESTART = 512
@@ -36,7 +37,7 @@ PROF_FAMILIES = ("spmv", "multidot", "update", "store", "xupdate", "residual", "
 class Params(C.Structure):
     _fields_ = [("restart", C.c_int32), ("max_iters", C.c_int32), ("format", C.c_int32), ("reorth", C.c_int32),
                 ("rel_tol", C.c_double), ("eta", C.c_double), ("h_res_history", C.c_void_p),
-                ("res_history_cap", C.c_int32), ("reserved", C.c_int32)]
+                ("res_history_cap", C.c_int32), ("precond", C.c_int32)]
 
 
 class Result(C.Structure):
@@ -189,9 +190,9 @@ class Solver:
             t = torch.as_tensor(np.ascontiguousarray(a), dtype=dtype, device=self.device)
         return t.contiguous()
 
-    def _params(self, restart, rel_tol, max_iters, fmt, reorth, eta, hist=None) -> Params:
+    def _params(self, restart, rel_tol, max_iters, fmt, reorth, eta, hist=None, precond="none") -> Params:
         p = Params(int(restart), int(max_iters), FORMAT_CODE[fmt], REORTH_CODE[reorth], float(rel_tol), float(eta),
-                   None, 0, 0)
+                   None, 0, PRECOND_CODE[precond])
         if hist is not None:
             p.h_res_history = hist.ctypes.data
             p.res_history_cap = hist.shape[0]
@@ -214,21 +215,22 @@ class Solver:
         self._keep = [rp, ci, va]  # BORROWED by the library until the next set_matrix / destroy
         self._check(self.lib.cbgmres_set_matrix(self.h, self.n, self.nnz, _ptr(rp), _ptr(ci), _ptr(va)))
 
-    def workspace_bytes(self, restart, fmt, history_cap=0) -> int:
+    def workspace_bytes(self, restart, fmt, history_cap=0, precond="none") -> int:
         hist = np.empty(history_cap) if history_cap else None
-        p = self._params(restart, 0.0, 0, fmt, "cond", 0.0, hist)
+        p = self._params(restart, 0.0, 0, fmt, "cond", 0.0, hist, precond)
         out = C.c_size_t(0)
         self._check(self.lib.cbgmres_workspace_bytes(self.h, C.byref(p), C.byref(out)))
         return int(out.value)
 
     def solve(self, b, x0, restart: int, rel_tol: float, max_iters: int, fmt: str = "fp64", reorth: str = "cond",
-              eta: float = 0.0, history: bool = False):
-        """Returns (x device tensor, SolveResult).  x0 is not modified."""
+              eta: float = 0.0, history: bool = False, precond: str = "none"):
+        """Returns (x device tensor, SolveResult).  x0 is not modified.  precond = "jacobi": right
+        preconditioner M = diag(A)."""
         torch = _torch()
         bt = self._dev(b, torch.float64)
         xt = self._dev(x0, torch.float64).clone()
         hist = np.full(max(int(max_iters), 1), np.nan) if history else None
-        p = self._params(restart, rel_tol, max_iters, fmt, reorth, eta, hist)
+        p = self._params(restart, rel_tol, max_iters, fmt, reorth, eta, hist, precond)
         need = C.c_size_t(0)
         self._check(self.lib.cbgmres_workspace_bytes(self.h, C.byref(p), C.byref(need)))
         ws = self._workspace(need.value)
@@ -238,13 +240,13 @@ class Solver:
         return xt, self._result(rc, res, hist)
 
     def solve_host(self, row_ptr, col_idx, vals, b, x, restart, rel_tol, max_iters, fmt="fp64", reorth="cond",
-                   eta=0.0):
+                   eta=0.0, precond="none"):
         """End-to-end call with HOST buffers (numpy arrays or pinned CPU tensors); x is overwritten."""
         def hp(a):
             return C.c_void_p(a.data_ptr()) if hasattr(a, "data_ptr") else C.c_void_p(a.ctypes.data)
 
         n, nnz = len(row_ptr) - 1, len(col_idx)
-        p = self._params(restart, rel_tol, max_iters, fmt, reorth, eta)
+        p = self._params(restart, rel_tol, max_iters, fmt, reorth, eta, None, precond)
         need = C.c_size_t(0)
         self._check(self.lib.cbgmres_workspace_bytes_host(self.h, n, nnz, C.byref(p), C.byref(need)))
         ws = self._workspace(need.value)

@@ -107,6 +107,9 @@ int launch_backsolve(cudaStream_t s, const Scratch &sc, const CycleState &cyc, i
 int launch_scale_coeffs(cudaStream_t s, int k, const double *h, const double *scales, double *hs);
 int launch_copy_scalars(cudaStream_t s, const double *src0, double *dst0, const double *src1, double *dst1);
 
+int launch_jacobi_setup(cudaStream_t s, const CsrView &A, double *d, double *scaled_vals); // d = diag(A), vals / d[col]
+int launch_diag_scale(cudaStream_t s, int64_t n, double *x, const double *d, int inverse);  // x *= d or x /= d
+
 int launch_row_stats(cudaStream_t s, int64_t n, const int32_t *d_row_ptr, int *d_out);
 
 // row-partition metadata for the streaming SpMV (set_matrix)

@@ -79,4 +79,48 @@ int launch_copy_scalars(cudaStream_t s, const double *src0, double *dst0, const 
     return 1;
 }
 
+// ---- scalar Jacobi right preconditioner M = diag(A) (Fig. 1 l.3 and l.17) ---------------
+// Applied by a change of variable, at no cost inside the Arnoldi loop: GMRES runs on A D^-1 (a
+// column-scaled copy of the values, made once per solve in the caller's workspace) in the variable
+// u = D x; the residual b - (A D^-1) u = b - A x is that of the original system, so every stopping
+// test is unchanged, and x = D^-1 u is formed once at the end.
+__global__ void jacobi_diag_kernel(int64_t n, const int32_t *__restrict__ rp, const int32_t *__restrict__ ci,
+                                   const double *__restrict__ va, double *__restrict__ d)
+{
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        double di = 1.0; // a row without a (nonzero) diagonal entry stays unscaled
+        for (int32_t p = rp[i]; p < rp[i + 1]; ++p)
+            if (ci[p] == i && va[p] != 0.0) di = va[p];
+        d[i] = di;
+    }
+}
+
+__global__ void jacobi_scale_vals_kernel(int64_t n, const int32_t *__restrict__ rp, const int32_t *__restrict__ ci,
+                                         const double *__restrict__ va, const double *__restrict__ d, double *__restrict__ out)
+{
+    const int64_t nnz = rp[n];
+    for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < nnz; p += (int64_t)gridDim.x * blockDim.x)
+        out[p] = va[p] / d[ci[p]];
+}
+
+// x_i *= d_i (inverse = 0) or x_i /= d_i (inverse = 1)
+__global__ void diag_scale_kernel(int64_t n, double *__restrict__ x, const double *__restrict__ d, int inverse)
+{
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        x[i] = inverse ? x[i] / d[i] : x[i] * d[i];
+}
+
+int launch_jacobi_setup(cudaStream_t s, const CsrView &A, double *d, double *scaled_vals)
+{
+    jacobi_diag_kernel<<<kNumSMs * 8, 256, 0, s>>>(A.n, A.row_ptr, A.col_idx, A.vals, d);
+    jacobi_scale_vals_kernel<<<kNumSMs * 8, 256, 0, s>>>(A.n, A.row_ptr, A.col_idx, A.vals, d, scaled_vals);
+    return 2;
+}
+
+int launch_diag_scale(cudaStream_t s, int64_t n, double *x, const double *d, int inverse)
+{
+    diag_scale_kernel<<<kNumSMs * 8, 256, 0, s>>>(n, x, d, inverse);
+    return 1;
+}
+
 } // namespace cbg

@@ -99,9 +99,10 @@ struct Layout {
     int64_t ld;
     size_t off_V, off_v, off_w, off_small, total;
     size_t o_h, o_hs, o_R, o_cs, o_sn, o_g, o_y, o_scales, o_hist;
+    size_t off_pvals, off_pdiag; // Jacobi: column-scaled values and diag(A) (unused otherwise)
 };
 
-Layout make_layout(int64_t n, const cbgmres_params *p)
+Layout make_layout(int64_t n, int64_t nnz, const cbgmres_params *p)
 {
     Layout L{};
     const int m = p->restart;
@@ -114,6 +115,12 @@ Layout make_layout(int64_t n, const cbgmres_params *p)
     o += up256((size_t)L.ld * 8);
     L.off_w = o;
     o += up256((size_t)L.ld * 8);
+    if (p->precond == CBGMRES_PRECOND_JACOBI) {
+        L.off_pvals = o;
+        o += up256((size_t)nnz * 8);
+        L.off_pdiag = o;
+        o += up256((size_t)n * 8);
+    }
     L.off_small = o;
     size_t s = 0;
     auto take = [&](size_t count) {
@@ -144,6 +151,8 @@ int validate_params(cbgmres_ctx *h, const cbgmres_params *p)
     if (!(p->rel_tol >= 0.0)) return fail(h, CBGMRES_E_INVALID, "rel_tol must be >= 0");
     if (!(p->eta >= 0.0) || p->eta > 1.0) return fail(h, CBGMRES_E_INVALID, "eta must be in [0, 1]");
     if (p->res_history_cap < 0) return fail(h, CBGMRES_E_INVALID, "res_history_cap < 0");
+    if (p->precond != CBGMRES_PRECOND_NONE && p->precond != CBGMRES_PRECOND_JACOBI)
+        return fail(h, CBGMRES_E_INVALID, "unknown preconditioner");
     return CBGMRES_OK;
 }
 
@@ -366,7 +375,7 @@ int cbgmres_workspace_bytes(cbgmres_handle_t h, const cbgmres_params *p, size_t 
     if (!h->has_matrix) return fail(h, CBGMRES_E_NOMATRIX, "set_matrix has not been called");
     const int rc = validate_params(h, p);
     if (rc) return rc;
-    *bytes = make_layout(h->A.n, p).total;
+    *bytes = make_layout(h->A.n, h->A.nnz, p).total;
     return CBGMRES_OK;
 }
 
@@ -384,7 +393,7 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
     if (reinterpret_cast<uintptr_t>(d_b) % 16 != 0 || reinterpret_cast<uintptr_t>(d_x) % 16 != 0)
         return fail(h, CBGMRES_E_INVALID, "b and x must be 16-byte aligned");
     const int64_t n = h->A.n;
-    const Layout L = make_layout(n, p);
+    const Layout L = make_layout(n, h->A.nnz, p);
     if (workspace_bytes < L.total) return fail(h, CBGMRES_E_WORKSPACE, "workspace too small");
     CK(cudaSetDevice(h->device));
     cudaStream_t s = h->stream;
@@ -442,6 +451,17 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
     }
     if (!std::isfinite(bnorm)) return fail(h, CBGMRES_E_NONFINITE, "||b|| is not finite");
 
+    // Scalar Jacobi: GMRES on A D^-1 in u = D x (small.cu); d_x holds u until the end
+    const bool jacobi = p->precond == CBGMRES_PRECOND_JACOBI;
+    CsrView A = h->A;
+    double *pdiag = nullptr;
+    if (jacobi) {
+        double *pvals = reinterpret_cast<double *>(ws + L.off_pvals);
+        pdiag = reinterpret_cast<double *>(ws + L.off_pdiag);
+        h->launches += launch_jacobi_setup(s, h->A, pdiag, pvals);
+        h->launches += launch_diag_scale(s, n, d_x, pdiag, 0);
+        A.vals = pvals;
+    }
     volatile int *flag = h->h_flag;
     const double dn = (double)n, dB = (double)B;
     const double bytes_spmv = 12.0 * (double)h->A.nnz + 4.0 * (dn + 1.0) + 16.0 * dn;
@@ -454,7 +474,7 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
         h->prof_on = h->opt_profile != 0;
         // l.1: r0 = b - A x, beta, the stopping test on the explicit residual; v1 = r0 / beta
         prof_begin(h, CBGMRES_PROF_RESIDUAL, 0, 0, bytes_spmv + 8.0 * dn + bytes_store);
-        h->launches += launch_spmv(s, h->sc, h->A, d_x, d_b, w, MODE_RESIDUAL, 0, &cy, h->d_flag);
+        h->launches += launch_spmv(s, h->sc, A, d_x, d_b, w, MODE_RESIDUAL, 0, &cy, h->d_flag);
         h->launches += launch_store(s, h->sc, fmt, n, w, &dctl->hn, &dctl->amax, 0.0, 0.0, Vp, cy.scales, v,
                                     MODE_RESIDUAL, 1, nullptr, nullptr);
         prof_end(h);
@@ -464,7 +484,7 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
             const double bytes_dot = (double)j * dn * dB + 8.0 * dn, bytes_upd = (double)j * dn * dB + 16.0 * dn;
             // l.3-4: w = A v, omega = ||w||
             prof_begin(h, CBGMRES_PROF_SPMV, j, 0, bytes_spmv);
-            h->launches += launch_spmv(s, h->sc, h->A, v, nullptr, w, MODE_STEP, j, nullptr, nullptr);
+            h->launches += launch_spmv(s, h->sc, A, v, nullptr, w, MODE_STEP, j, nullptr, nullptr);
             prof_end(h);
             // l.5: h = V^T w
             prof_begin(h, CBGMRES_PROF_MULTIDOT, j, 1, bytes_dot);
@@ -512,7 +532,10 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
         CK(cudaMemcpyAsync(h->h_ctl, dctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
         CK(cudaStreamSynchronize(s));
         CK(cudaGetLastError());
-        if (take_orth_error()) return fail(h, CBGMRES_E_CUDA, "cuTensorMapEncodeTiled failed for the basis");
+        if (take_orth_error()) {
+            if (jacobi) launch_diag_scale(s, n, d_x, pdiag, 1);
+            return fail(h, CBGMRES_E_CUDA, "cuTensorMapEncodeTiled failed for the basis");
+        }
         if (h->opt_profile) {
             const bool cycle_ran = h->h_ctl->restarts > restarts_before;
             // the x update's bytes depend on k, known only now
@@ -523,6 +546,7 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
         }
         if (h->h_ctl->done) break;
     }
+    if (jacobi) h->launches += launch_diag_scale(s, n, d_x, pdiag, 1); // l.17: x = M^-1 u
     if (hist_cap) {
         const int cnt = h->h_ctl->iters < hist_cap ? h->h_ctl->iters : hist_cap;
         if (cnt > 0) CK(cudaMemcpyAsync(p->h_res_history, cy.hist, (size_t)cnt * 8, cudaMemcpyDeviceToHost, s));
@@ -552,7 +576,7 @@ int cbgmres_workspace_bytes_host(cbgmres_handle_t h, int64_t n, int64_t nnz, con
     if (rc) return rc;
     if (n <= 0 || nnz < 0) return fail(h, CBGMRES_E_INVALID, "bad n / nnz");
     *bytes = up256((size_t)(n + 1) * 4) + up256((size_t)nnz * 4) + up256((size_t)nnz * 8) + 2 * up256((size_t)n * 8) +
-             make_layout(n, p).total;
+             make_layout(n, nnz, p).total;
     return CBGMRES_OK;
 }
 

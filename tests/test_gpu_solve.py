@@ -11,14 +11,15 @@ from workloads import make_config, random_dense_system
 pytestmark = pytest.mark.gpu
 
 
-def _solve_gpu(p, fmt, restart=None, rel_tol=None, max_iters=None, reorth="cond", history=False, x0=None):
+def _solve_gpu(p, fmt, restart=None, rel_tol=None, max_iters=None, reorth="cond", history=False, x0=None,
+               precond="none"):
     from paper_2009_12101_b200 import Solver
 
     s = Solver(0)
     try:
         s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
         x, r = s.solve(p.b, p.x0 if x0 is None else x0, restart or p.restart, rel_tol or p.rel_tol,
-                       max_iters or p.max_iters, fmt, reorth=reorth, history=history)
+                       max_iters or p.max_iters, fmt, reorth=reorth, history=history, precond=precond)
         return x.cpu().numpy(), r
     finally:
         s.destroy()
@@ -28,7 +29,7 @@ def _true_rel_res(p, x):
     return oracle.nrm2(p.b - oracle.spmv(p.A, x)) / oracle.nrm2(p.b)
 
 
-def _assert_iters_parity(gpu_iters, ref, p, fmt, restart, rel_tol, max_iters, reorth):
+def _assert_iters_parity(gpu_iters, ref, p, fmt, restart, rel_tol, max_iters, reorth, precond="none"):
     """+-2 % (at least +-2 steps) of the oracle's iteration count.  With a quantised basis the store
     is a discontinuous map: a last-bit difference in one inner product flips rounding decisions and
     the two residual histories decorrelate at the level of the storage format's unit roundoff after
@@ -44,21 +45,22 @@ def _assert_iters_parity(gpu_iters, ref, p, fmt, restart, rel_tol, max_iters, re
     try:
         for t in (1, 2, 3, 5):
             oracle.set_num_threads(t)
-            counts.append(oracle.gmres(p.A, p.b, p.x0, restart, rel_tol, max_iters, fmt, reorth=reorth).iters)
+            counts.append(oracle.gmres(p.A, p.b, p.x0, restart, rel_tol, max_iters, fmt, reorth=reorth,
+                                       precond=precond).iters)
     finally:
         oracle.set_num_threads(base)
     lo, hi = min(counts), max(counts)
     assert lo - tol(lo) <= gpu_iters <= hi + tol(hi), (fmt, gpu_iters, counts)
 
 
-def _check_parity(p, fmt, restart=None, rel_tol=None, max_iters=None, reorth="cond"):
+def _check_parity(p, fmt, restart=None, rel_tol=None, max_iters=None, reorth="cond", precond="none"):
     restart, rel_tol, max_iters = restart or p.restart, rel_tol or p.rel_tol, max_iters or p.max_iters
-    ref = oracle.gmres(p.A, p.b, p.x0, restart, rel_tol, max_iters, fmt, reorth=reorth)
-    x, r = _solve_gpu(p, fmt, restart, rel_tol, max_iters, reorth)
+    ref = oracle.gmres(p.A, p.b, p.x0, restart, rel_tol, max_iters, fmt, reorth=reorth, precond=precond)
+    x, r = _solve_gpu(p, fmt, restart, rel_tol, max_iters, reorth, precond=precond)
     true_gpu = _true_rel_res(p, x)
     true_ref = _true_rel_res(p, ref.x)
     assert r.converged == ref.converged
-    _assert_iters_parity(r.iters, ref, p, fmt, restart, rel_tol, max_iters, reorth)
+    _assert_iters_parity(r.iters, ref, p, fmt, restart, rel_tol, max_iters, reorth, precond)
     if ref.converged:
         assert true_gpu <= rel_tol * (1 + 1e-9) and true_ref <= rel_tol * (1 + 1e-9)
     assert true_gpu <= 10 * true_ref and true_ref <= 10 * true_gpu
@@ -86,6 +88,59 @@ def test_c4_reduced(fmt):
     # sides must then stop at the bound with comparable true residuals
     r, ref = _check_parity(make_config("C4", n=40000), fmt, max_iters=300)
     assert r.iters == ref.iters == 300
+
+
+@pytest.mark.parametrize("fmt", oracle.FORMATS)
+def test_c4_reduced_jacobi_converges(fmt):
+    """The paper's default preconditioner (scalar Jacobi) as the right preconditioner of
+    Fig. 1 l.3 / l.17: C4 converges on both sides, counts and residuals as in every other parity case."""
+    r, ref = _check_parity(make_config("C4", n=40000), fmt, max_iters=2000, precond="jacobi")
+    assert r.converged and ref.converged
+
+
+@pytest.mark.parametrize("fmt", ["fp64", "fp16"])
+def test_c2_reduced_jacobi_constant_diagonal(fmt):
+    """C2's diagonal is the constant 6: A D^-1 = A / 6, same Krylov spaces (streamed SpMV variant with
+    the scaled copy of the values; x = D^-1 u at the end)."""
+    p = make_config("C2", grid=32)
+    r, ref = _check_parity(p, fmt, precond="jacobi")
+    _, plain = _solve_gpu(p, fmt)
+    assert r.converged and abs(r.iters - plain.iters) <= max(2, 0.02 * plain.iters)
+
+
+def test_jacobi_tiny_dense_nonzero_x0_matches_direct_solve():
+    A, Ad, b = random_dense_system(48, 61, density=0.4)
+    col = 10.0 ** np.random.default_rng(62).uniform(-2.0, 2.0, 48)
+    col[::3] *= -1.0
+    import scipy.sparse as sp
+    from workloads import CSR, Problem
+
+    S = sp.csr_matrix(Ad * col[None, :])
+    S.sort_indices()
+    A2 = CSR(48, S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(np.float64))
+    x0 = np.random.default_rng(63).standard_normal(48)
+    p = Problem("tiny", A2, b, x0, 48, 1e-12, 400, ("fp64",), {})
+    x, r = _solve_gpu(p, "fp64", precond="jacobi")
+    xs = np.linalg.solve(Ad * col[None, :], b)
+    assert r.converged
+    assert np.linalg.norm(x - xs) <= 1e-8 * np.linalg.norm(xs)
+    assert _true_rel_res(p, x) <= 1e-12 * (1 + 1e-6)
+
+
+def test_jacobi_host_entry_and_workspace():
+    """solve_host with the preconditioner: the extra workspace (scaled values + diagonal) is accounted for."""
+    from paper_2009_12101_b200 import Solver
+
+    p = make_config("C4", n=20000)
+    s = Solver(0)
+    try:
+        x = p.x0.copy()
+        r = s.solve_host(p.A.row_ptr, p.A.col_idx, p.A.vals, p.b, x, p.restart, p.rel_tol, 2000, "fp32", precond="jacobi")
+        assert r.converged and _true_rel_res(p, x) <= p.rel_tol * (1 + 1e-6)
+        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+        assert s.workspace_bytes(p.restart, "fp32", precond="jacobi") >= s.workspace_bytes(p.restart, "fp32") + 8 * (p.A.nnz + p.A.n)
+    finally:
+        s.destroy()
 
 
 @pytest.mark.parametrize("fmt", oracle.FORMATS)
