@@ -213,6 +213,25 @@ __device__ __forceinline__ double ldg_stream_f64(const double *p, uint64_t pol)
     return r;
 }
 
+// Gather of one entry of x by the streaming kernel.  Random columns find nothing in L1 (x is 16 MB), so
+// the gathers go to L2 directly (ld.global.cg): C4, n = 2e6: 387 -> 369 us against ld.global.nc through
+// L1; the .L1::no_allocate form of the nc load was far slower (545 us).  -DCBG_GATHER=0 / 2 select those.
+#ifndef CBG_GATHER
+#define CBG_GATHER 1
+#endif
+__device__ __forceinline__ double gather_x(const double *p)
+{
+#if CBG_GATHER == 1
+    return __ldcg(p);
+#elif CBG_GATHER == 2
+    double r;
+    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(r) : "l"(p));
+    return r;
+#else
+    return __ldg(p);
+#endif
+}
+
 __global__ void __launch_bounds__(kStreamThreads) spmv_stream_kernel(const SpmvArgs a)
 {
     pdl_wait();
@@ -250,7 +269,7 @@ __global__ void __launch_bounds__(kStreamThreads) spmv_stream_kernel(const SpmvA
                 }
                 double xv[kStreamItems];
 #pragma unroll
-                for (int i = 0; i < kStreamItems; ++i) xv[i] = __ldg(x + c[i]);
+                for (int i = 0; i < kStreamItems; ++i) xv[i] = gather_x(x + c[i]);
 #pragma unroll
                 for (int i = 0; i < kStreamItems; ++i) {
                     const int q = off + i * kStreamThreads + tid;
