@@ -84,3 +84,35 @@ def test_bytes_model_against_survey_table():
     assert model.store_bytes(n, "fp64") == 24 * n and model.store_bytes(n, "int16") == 18 * n
     assert model.arnoldi_step_bytes(n, nnz, 10, "fp32", reorth=True) - model.arnoldi_step_bytes(n, nnz, 10, "fp32") \
         == model.multidot_bytes(n, 10, "fp32") + model.update_bytes(n, 10, "fp32")
+
+
+def test_cycle_bytes_model_has_the_papers_asymptotes():
+    """the per-cycle speedup of a 32-bit (16-bit) basis approaches a value below 2x (4x) as
+    the restart length grows, because the SpMV and the vector traffic do not shrink.  The algorithmic
+    bytes model of cyclebench.py must show exactly that."""
+    from paper_2009_12101_b200.cyclebench import cycle_bytes
+
+    n, nnz = 1_000_000, 6_940_000
+    prev32 = prev16 = 1.0
+    for m in (10, 50, 100, 300, 3000):
+        r32 = cycle_bytes(n, nnz, m, "fp64", 0.0) / cycle_bytes(n, nnz, m, "fp32", 0.0)
+        r16 = cycle_bytes(n, nnz, m, "fp64", 0.0) / cycle_bytes(n, nnz, m, "int16", 0.0)
+        assert prev32 < r32 < 2.0 and prev16 < r16 < 4.0 and r16 > r32
+        prev32, prev16 = r32, r16
+    assert prev32 > 1.98 and prev16 > 3.9
+    # re-orthogonalised steps read the basis three times instead of two (DESIGN.md section 6)
+    m, B = 100, 4
+    extra = cycle_bytes(n, nnz, m, "fp32", 1.0) - cycle_bytes(n, nnz, m, "fp32", 0.0)
+    assert extra == sum(j * n * B + 16 * n for j in range(1, m + 1))
+    assert cycle_bytes(n, nnz, m, "fp32", 0.0) == cycle_bytes(n, nnz, m, "int32", 0.0)
+
+
+def test_paper_protocol_matrix_set_uses_known_configs():
+    from paper_2009_12101_b200 import paperprotocol
+    from workloads import make_config
+    from workloads.generators import CONFIG_NAMES
+
+    for label, cfg, kw in paperprotocol.MATRICES + paperprotocol.SMALL:
+        assert cfg in CONFIG_NAMES and set(kw) <= {"grid", "n"}
+    p = make_config(*paperprotocol.SMALL[0][1:2], **paperprotocol.SMALL[0][2])
+    assert p.A.n == 24 ** 3
