@@ -46,12 +46,13 @@ def main(argv=None) -> int:
     ap.add_argument("--formats", default=",".join(FORMATS))
     ap.add_argument("--reorth", default="cond")
     ap.add_argument("--json", default="")
+    ap.add_argument("--grid", type=int, default=0, help="shrink a stencil workload to grid^d points (same recipe)")
     args = ap.parse_args(argv)
     ms = [int(x) for x in args.m.split(",") if x]
     fmts = [f for f in args.formats.split(",") if f]
     if "fp64" not in fmts:
         fmts.insert(0, "fp64")
-    p = make_config(args.workload)
+    p = make_config(args.workload, **({"grid": args.grid} if args.grid else {}))
     n, nnz = p.A.n, p.A.nnz
     s = Solver(0)
     s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)

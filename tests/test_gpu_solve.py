@@ -287,3 +287,17 @@ def test_full_size_c2_solve_is_bitwise_repeatable(fmt):
             assert np.array_equal(x, runs[0][0])
     finally:
         s.destroy()
+
+
+def test_measurement_drivers_run(capsys):
+    """cyclebench (fixed iteration count: every solve does exactly cycles * m steps) and paperprotocol
+    (b_i = sin i, Jacobi) on small inputs."""
+    from paper_2009_12101_b200 import cyclebench, paperprotocol
+
+    assert cyclebench.main(["--workload", "C2", "--grid", "20", "--m", "5,12", "--cycles", "3", "--formats", "fp64,int16"]) == 0
+    out = capsys.readouterr().out
+    rows = [l.split() for l in out.splitlines() if l and l[0] == " " and l.split()[0].isdigit()]
+    assert [(int(r[0]), r[1], int(r[2])) for r in rows] == [(5, "fp64", 15), (5, "int16", 15), (12, "fp64", 36), (12, "int16", 36)]
+    assert paperprotocol.main(["--small", "--max-iters", "3000"]) == 0
+    out = capsys.readouterr().out
+    assert "fp32" in out and "3/3" in out
