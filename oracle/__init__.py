@@ -36,7 +36,8 @@ class _Result(C.Structure):
 
 class _Capture(C.Structure):
     _fields_ = [("cycle", C.c_int32), ("k", C.c_int32), ("beta", C.c_double), ("Vhat", C.c_void_p),
-                ("Vfp64", C.c_void_p), ("Hbar", C.c_void_p), ("y", C.c_void_p), ("g", C.c_void_p)]
+                ("Vfp64", C.c_void_p), ("Hbar", C.c_void_p), ("y", C.c_void_p), ("g", C.c_void_p),
+                ("reorth_log", C.c_void_p), ("omega", C.c_void_p)]
 
 
 def lib():
@@ -74,6 +75,14 @@ def lib():
         L.orc_gmres_m.restype = C.c_int
         L.orc_jacobi_diag.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_jacobi_diag.restype = None
+        L.orc_block_jacobi4.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_block_jacobi4.restype = None
+        L.orc_apply_minv.argtypes = [C.c_int, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+        L.orc_apply_minv.restype = None
+        L.orc_gmres_p.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p,
+                                  C.c_void_p, C.POINTER(_Params), C.POINTER(_Result), C.c_void_p, C.c_int32, C.c_void_p,
+                                  C.c_int32, C.POINTER(_Capture)]
+        L.orc_gmres_p.restype = C.c_int
         _lib = L
     return _lib
 
@@ -199,11 +208,31 @@ def jacobi_diag(A) -> np.ndarray:
     return d
 
 
+PRECOND_CODE = {"none": 0, "jacobi": 1, "block_jacobi4": 2}
+
+
+def block_jacobi4(A) -> np.ndarray:
+    """The inverted 4 x 4 diagonal blocks of A, [ceil(n/4), 4, 4] (orc_block_jacobi4)."""
+    inv = np.empty(((A.n + 3) // 4, 4, 4))
+    lib().orc_block_jacobi4(A.n, _p(A.row_ptr), _p(A.col_idx), _p(A.vals), _p(inv))
+    return inv
+
+
+def apply_minv(precond: str, pdata, v) -> np.ndarray:
+    """z = M^-1 v as the solver applies it in Fig. 1 l.3 / l.17 (pdata: jacobi_diag / block_jacobi4 output)."""
+    v = _f64(v)
+    z = np.empty_like(v)
+    pd = _f64(pdata) if pdata is not None else None
+    lib().orc_apply_minv(PRECOND_CODE[precond], _p(pd) if pd is not None else None, v.shape[0], _p(v), _p(z))
+    return z
+
+
 def gmres(A, b, x0, restart: int, rel_tol: float, max_iters: int, fmt: str = "fp64", reorth: str = "cond",
           eta: float = 1.0 / math.sqrt(2.0), capture_cycle: int | None = None, precond: str = "none") -> OracleResult:
-    """Restarted CB-GMRES (Fig. 1).  See orc_gmres_m in cbgmres_oracle.c.
-    precond = "jacobi": right preconditioner M = diag(A) (Fig. 1 l.3 and l.17)."""
-    if precond not in ("none", "jacobi"):
+    """Restarted CB-GMRES (Fig. 1).  See orc_gmres_p in cbgmres_oracle.c.
+    precond = "jacobi": right preconditioner M = diag(A) (PAPER.md:186; Fig. 1 l.3 and l.17);
+    precond = "block_jacobi4": M = the 4 x 4 diagonal blocks of A."""
+    if precond not in PRECOND_CODE:
         raise ValueError(precond)
     b = _f64(b)
     x = _f64(x0).copy()
@@ -216,10 +245,12 @@ def gmres(A, b, x0, restart: int, rel_tol: float, max_iters: int, fmt: str = "fp
     bufs = {}
     if capture_cycle is not None:
         bufs = dict(Vhat=np.zeros((m + 1, n)), Vfp64=np.zeros((m + 1, n)), Hbar=np.zeros((m, m + 1)),
-                    y=np.zeros(m), g=np.zeros(m + 1))
-        cap = _Capture(capture_cycle, 0, 0.0, *[bufs[k].ctypes.data for k in ("Vhat", "Vfp64", "Hbar", "y", "g")])
-    mdiag = jacobi_diag(A) if precond == "jacobi" else None
-    rc = lib().orc_gmres_m(n, _p(A.row_ptr), _p(A.col_idx), _p(A.vals), _p(mdiag) if mdiag is not None else None,
+                    y=np.zeros(m), g=np.zeros(m + 1), reorth_log=np.zeros(m, dtype=np.int32), omega=np.zeros(m))
+        cap = _Capture(capture_cycle, 0, 0.0, *[bufs[k].ctypes.data for k in ("Vhat", "Vfp64", "Hbar", "y", "g",
+                                                                              "reorth_log", "omega")])
+    pdata = jacobi_diag(A) if precond == "jacobi" else block_jacobi4(A) if precond == "block_jacobi4" else None
+    rc = lib().orc_gmres_p(n, _p(A.row_ptr), _p(A.col_idx), _p(A.vals), PRECOND_CODE[precond],
+                           _p(pdata) if pdata is not None else None,
                            _p(b), _p(x), C.byref(prm), C.byref(res), _p(rec), rec.shape[0], _p(expl), expl.shape[0],
                            C.byref(cap) if cap else None)
     if rc != 0:
@@ -228,7 +259,8 @@ def gmres(A, b, x0, restart: int, rel_tol: float, max_iters: int, fmt: str = "fp
     if cap is not None:
         k = cap.k
         capture = dict(k=k, beta=cap.beta, Vhat=bufs["Vhat"][: k + 1], Vfp64=bufs["Vfp64"][: k + 1],
-                       Hbar=bufs["Hbar"].T[: k + 1, :k].copy(), y=bufs["y"][:k], g=bufs["g"][: k + 1])
+                       Hbar=bufs["Hbar"].T[: k + 1, :k].copy(), y=bufs["y"][:k], g=bufs["g"][: k + 1],
+                       reorth_log=bufs["reorth_log"][:k].copy(), omega=bufs["omega"][:k].copy())
     return OracleResult(x, res.iters, res.restarts, res.reorth_count, res.breakdown, bool(res.converged),
                         res.rel_res_recurrence, res.rel_res_true, res.b_norm, rec[: res.iters],
                         expl[~np.isnan(expl)], capture)

@@ -20,6 +20,11 @@
  *   - GMRES (compressed storage): mixed Arnoldi relation, |V^| <= 1, explicit residual <= tol.
  *   - right preconditioner M = diag(A) (orc_gmres_m): numpy.linalg.solve on badly scaled systems,
  *     residual history equal to plain GMRES on the explicitly formed A D^-1, constant-diagonal no-op.
+ *   - right preconditioner M = blockdiag_4(A) (orc_block_jacobi4, orc_gmres_p): every inverted
+ *     block against numpy.linalg.inv, numpy.linalg.solve on dense systems, residual history equal to plain
+ *     GMRES on the explicitly formed A M^-1, reduction to scalar Jacobi for block-diagonal-free matrices.
+ *   - Fig. 1 l.12 (second-pass breakdown, reading Q4): a matrix with an exact invariant subspace and a
+ *     quantised basis, where the clause hn < eta * omega1 -- and not hn == 0 -- ends the cycle.
  *   - PARITY UNPINNED: exact iteration counts of the compressed formats on the synthetic configs
  *     (the paper prints no value for any of them; only Table 2's qualitative ratios apply).
  *
@@ -380,6 +385,8 @@ typedef struct {      /* optional capture of one restart cycle, for the pins */
     double *Hbar;     /* out: (m+1) x m, column-major, the UNROTATED Hessenberg matrix (l.16) */
     double *y;        /* out: m, the minimiser of l.17 */
     double *g;        /* out: m+1, rotated right-hand side at the end of the cycle */
+    int32_t *reorth_log; /* out: m, 1 where l.7 fired at that step of the cycle (may be NULL) */
+    double *omega;    /* out: m, omega = ||A M^-1 v_j||_2 of l.4 at that step (may be NULL) */
 } orc_capture;
 
 /* Scalar Jacobi preconditioner M = diag(A) ("a scalar Jacobi preconditioner" in every
@@ -393,22 +400,102 @@ void orc_jacobi_diag(int64_t n, const int32_t *rp, const int32_t *ci, const doub
     }
 }
 
-/* Fig. 1 with a right preconditioner M = diag(mdiag) (mdiag == NULL: M = I):
+/* Block-Jacobi preconditioner with blocks of size 4 (section 6.5: "a block-Jacobi
+ * preconditioning scheme with block-size 4"), fixed (fp64) precision: M = blockdiag(A_00, A_11, ...),
+ * A_bb = rows and columns 4b .. 4b+3 of A (entries absent from the pattern are 0; the last block has
+ * n mod 4 rows when 4 does not divide n and is completed by the identity).  Each block is inverted
+ * by plain Gaussian elimination with partial pivoting on [A_bb | I] (Gauss-Jordan); a block that turns
+ * out singular (a zero pivot column) is replaced by the identity, as the scalar variant leaves a row
+ * with a zero diagonal unscaled.  inv[16 b + 4 r + c] = (A_bb^-1)_{rc}. */
+void orc_block_jacobi4(int64_t n, const int32_t *rp, const int32_t *ci, const double *va, double *inv)
+{
+    const int64_t nb = (n + 3) / 4;
+    for (int64_t b = 0; b < nb; b++) {
+        double a[4][8];
+        for (int r = 0; r < 4; r++)
+            for (int c = 0; c < 8; c++) a[r][c] = (c == r + 4) ? 1.0 : 0.0;
+        for (int r = 0; r < 4; r++) {
+            const int64_t i = 4 * b + r;
+            if (i >= n) { a[r][r] = 1.0; continue; } /* ragged last block: identity */
+            for (int32_t p = rp[i]; p < rp[i + 1]; p++) {
+                const int64_t c = (int64_t)ci[p] - 4 * b;
+                if (c >= 0 && c < 4) a[r][c] += va[p];
+            }
+        }
+        int singular = 0;
+        for (int k = 0; k < 4 && !singular; k++) {
+            int piv = k;
+            for (int r = k + 1; r < 4; r++)
+                if (fabs(a[r][k]) > fabs(a[piv][k])) piv = r;
+            if (a[piv][k] == 0.0 || !isfinite(a[piv][k])) { singular = 1; break; }
+            if (piv != k)
+                for (int c = 0; c < 8; c++) { double t = a[k][c]; a[k][c] = a[piv][c]; a[piv][c] = t; }
+            const double d = a[k][k];
+            for (int c = 0; c < 8; c++) a[k][c] = a[k][c] / d;
+            for (int r = 0; r < 4; r++) {
+                if (r == k) continue;
+                const double f = a[r][k];
+                if (f == 0.0) continue;
+                for (int c = 0; c < 8; c++) a[r][c] = a[r][c] - f * a[k][c];
+            }
+        }
+        for (int r = 0; r < 4; r++)
+            for (int c = 0; c < 4; c++) inv[16 * b + 4 * r + c] = singular ? (r == c ? 1.0 : 0.0) : a[r][c + 4];
+    }
+}
+
+/* z := M^-1 v for the preconditioner kinds below (l.3 and l.17 of Fig. 1). */
+enum { ORC_PRECOND_NONE = 0, ORC_PRECOND_JACOBI = 1, ORC_PRECOND_BLOCK_JACOBI4 = 2 };
+static void apply_minv(int kind, const double *pdata, int64_t n, const double *v, double *z)
+{
+    int64_t i;
+    if (kind == ORC_PRECOND_JACOBI) { /* pdata = d, d_i = a_ii */
+#pragma omp parallel for schedule(static)
+        for (i = 0; i < n; i++) z[i] = v[i] / pdata[i];
+    } else if (kind == ORC_PRECOND_BLOCK_JACOBI4) { /* pdata = the inverted blocks of orc_block_jacobi4 */
+        const int64_t nb = (n + 3) / 4;
+#pragma omp parallel for schedule(static)
+        for (i = 0; i < nb; i++) {
+            for (int r = 0; r < 4; r++) {
+                if (4 * i + r >= n) break;
+                double s = 0.0;
+                for (int c = 0; c < 4; c++)
+                    if (4 * i + c < n) s += pdata[16 * i + 4 * r + c] * v[4 * i + c];
+                z[4 * i + r] = s;
+            }
+        }
+    } else {
+        memcpy(z, v, (size_t)n * 8);
+    }
+}
+void orc_apply_minv(int kind, const double *pdata, int64_t n, const double *v, double *z) { apply_minv(kind, pdata, n, v, z); }
+
+/* Fig. 1 with a right preconditioner M (kind = ORC_PRECOND_*, pdata as apply_minv reads it; kind 0: M = I):
  * l.3 "w := A (M^-1 v_j)" and l.17 "x_m := x_0 + M^-1 (V_m y_m)"; the residual
  * of l.1 and the stopping test are those of the ORIGINAL system A x = b (right preconditioning
  * leaves the residual unchanged). */
-int orc_gmres_m(int64_t n, const int32_t *rp, const int32_t *ci, const double *va, const double *mdiag,
+int orc_gmres_p(int64_t n, const int32_t *rp, const int32_t *ci, const double *va, int kind, const double *pdata,
                 const double *b, double *x, const orc_params *prm, orc_result *res, double *rec_hist,
                 int32_t rec_hist_cap, double *expl_hist, int32_t expl_hist_cap, orc_capture *cap);
+
+/* M = diag(mdiag) (mdiag == NULL: M = I). */
+int orc_gmres_m(int64_t n, const int32_t *rp, const int32_t *ci, const double *va, const double *mdiag,
+                const double *b, double *x, const orc_params *prm, orc_result *res, double *rec_hist,
+                int32_t rec_hist_cap, double *expl_hist, int32_t expl_hist_cap, orc_capture *cap)
+{
+    return orc_gmres_p(n, rp, ci, va, mdiag ? ORC_PRECOND_JACOBI : ORC_PRECOND_NONE, mdiag, b, x, prm, res, rec_hist,
+                       rec_hist_cap, expl_hist, expl_hist_cap, cap);
+}
 
 int orc_gmres(int64_t n, const int32_t *rp, const int32_t *ci, const double *va, const double *b, double *x,
               const orc_params *prm, orc_result *res, double *rec_hist, int32_t rec_hist_cap, double *expl_hist,
               int32_t expl_hist_cap, orc_capture *cap)
 {
-    return orc_gmres_m(n, rp, ci, va, NULL, b, x, prm, res, rec_hist, rec_hist_cap, expl_hist, expl_hist_cap, cap);
+    return orc_gmres_p(n, rp, ci, va, ORC_PRECOND_NONE, NULL, b, x, prm, res, rec_hist, rec_hist_cap, expl_hist,
+                       expl_hist_cap, cap);
 }
 
-int orc_gmres_m(int64_t n, const int32_t *rp, const int32_t *ci, const double *va, const double *mdiag,
+int orc_gmres_p(int64_t n, const int32_t *rp, const int32_t *ci, const double *va, int kind, const double *pdata,
                 const double *b, double *x, const orc_params *prm, orc_result *res, double *rec_hist,
                 int32_t rec_hist_cap, double *expl_hist, int32_t expl_hist_cap, orc_capture *cap)
 {
@@ -469,9 +556,8 @@ int orc_gmres_m(int64_t n, const int32_t *rp, const int32_t *ci, const double *v
         int k = 0, breakdown = 0;
         for (int j = 1; j <= m; j++) {
             /* l.3: w := A (M^-1 v)   (the fp64 v, reading Q1) */
-            if (mdiag) {
-#pragma omp parallel for schedule(static)
-                for (i = 0; i < n; i++) z[i] = v[i] / mdiag[i];
+            if (kind != ORC_PRECOND_NONE) {
+                apply_minv(kind, pdata, n, v, z);
                 orc_spmv(n, rp, ci, va, z, w);
             } else {
                 orc_spmv(n, rp, ci, va, v, w);
@@ -491,9 +577,12 @@ int orc_gmres_m(int64_t n, const int32_t *rp, const int32_t *ci, const double *v
             /* l.6: h_{j+1,j} := ||w||_2 */
             double hn = nrm2(n, w);
             breakdown = (hn == 0.0);
+            if (capture && cap->omega) cap->omega[j - 1] = omega;
+            if (capture && cap->reorth_log) cap->reorth_log[j - 1] = 0;
             /* l.7: if h_{j+1,j} < eta * omega then re-orthogonalise (one extra pass, reading Q3) */
             if (prm->reorth == ORC_REORTH_ALWAYS || (prm->reorth == ORC_REORTH_COND && hn < eta * omega)) {
                 const double omega1 = hn; /* norm before the second pass (reading Q4) */
+                if (capture && cap->reorth_log) cap->reorth_log[j - 1] = 1;
                 /* l.8: u := V_j^T w, w := w - V_j u */
                 for (int c = 0; c < j; c++) {
                     orc_dec(fmt, n, VCOL(c), sigma[c], tmp);
@@ -555,14 +644,23 @@ int orc_gmres_m(int64_t n, const int32_t *rp, const int32_t *ci, const double *v
             y[r] = s / R[(size_t)r * (m + 1) + r];
         }
         /*       x := x_0 + M^-1 (V_k y)   (decoded basis) */
-        if (mdiag) {
+        if (kind == ORC_PRECOND_JACOBI) {
             memset(z, 0, (size_t)n * 8);
             for (int c = 0; c < k; c++) {
                 orc_dec(fmt, n, VCOL(c), sigma[c], tmp);
                 axpy(n, y[c], tmp, z);
             }
 #pragma omp parallel for schedule(static)
-            for (i = 0; i < n; i++) x[i] += z[i] / mdiag[i];
+            for (i = 0; i < n; i++) x[i] += z[i] / pdata[i];
+        } else if (kind != ORC_PRECOND_NONE) {
+            memset(z, 0, (size_t)n * 8);
+            for (int c = 0; c < k; c++) {
+                orc_dec(fmt, n, VCOL(c), sigma[c], tmp);
+                axpy(n, y[c], tmp, z);
+            }
+            apply_minv(kind, pdata, n, z, tmp);
+#pragma omp parallel for schedule(static)
+            for (i = 0; i < n; i++) x[i] += tmp[i];
         } else {
             for (int c = 0; c < k; c++) {
                 orc_dec(fmt, n, VCOL(c), sigma[c], tmp);

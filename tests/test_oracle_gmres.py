@@ -299,3 +299,199 @@ def test_jacobi_makes_the_power_law_config_converge():
     assert np.linalg.norm(p.b - S @ j.x) <= p.rel_tol * np.linalg.norm(p.b) * (1 + 1e-6)
     a = oracle.gmres(p.A, p.b, p.x0, precond="none", **kw)
     assert (not a.converged) or a.iters > 2 * j.iters
+
+
+# ---- block-Jacobi right preconditioner, block size 4 (section 6.5) ---------------------------
+
+def _csr_from_dense(Ad):
+    from workloads import CSR
+    import scipy.sparse as sp
+
+    S = sp.csr_matrix(Ad)
+    S.sort_indices()
+    return CSR(Ad.shape[0], S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(np.float64))
+
+
+def _block_system(n, seed, coupling=0.05):
+    """Dense nonsymmetric system A = (I + coupling G) M with M block diagonal: strong, badly scaled 4 x 4
+    diagonal blocks (scales spanning two decades, a large ANTI-diagonal inside each block, so that
+    pivoting is needed and the scalar diagonal is a poor preconditioner) and weak coupling between the
+    blocks.  Input construction only."""
+    rng = np.random.default_rng(seed)
+    M = np.zeros((n, n))
+    for b0 in range(0, n, 4):
+        b1 = min(n, b0 + 4)
+        blk = 0.3 * rng.standard_normal((b1 - b0, b1 - b0)) + 2.0 * np.eye(b1 - b0)[::-1] + 0.5 * np.eye(b1 - b0)
+        M[b0:b1, b0:b1] = 10.0 ** rng.uniform(-1.0, 1.0) * blk
+    Ad = (np.eye(n) + coupling * rng.standard_normal((n, n))) @ M
+    b = rng.standard_normal(n)
+    return _csr_from_dense(Ad), Ad, b
+
+
+@pytest.mark.parametrize("n", [16, 18, 19, 3])
+def test_block_jacobi4_blocks_match_numpy_inv(n):
+    A, Ad, _ = _block_system(n, 80 + n)
+    inv = oracle.block_jacobi4(A)
+    assert inv.shape == ((n + 3) // 4, 4, 4)
+    for b in range(inv.shape[0]):
+        b0, b1 = 4 * b, min(n, 4 * b + 4)
+        s = b1 - b0
+        ref = np.linalg.inv(Ad[b0:b1, b0:b1])
+        assert np.allclose(inv[b, :s, :s], ref, rtol=1e-11, atol=1e-13 * np.abs(ref).max())
+        # ragged last block: completed by the identity, nothing couples into the real rows
+        assert np.array_equal(inv[b, s:, s:], np.eye(4 - s)) and not inv[b, :s, s:].any() and not inv[b, s:, :s].any()
+    # apply: z = M^-1 v block by block
+    v = np.random.default_rng(5).standard_normal(n)
+    z = oracle.apply_minv("block_jacobi4", inv, v)
+    M = np.zeros((n, n))
+    for b0 in range(0, n, 4):
+        b1 = min(n, b0 + 4)
+        M[b0:b1, b0:b1] = Ad[b0:b1, b0:b1]
+    assert np.allclose(z, np.linalg.solve(M, v), rtol=1e-10, atol=1e-13 * np.abs(z).max())
+
+
+def test_block_jacobi4_sparse_pattern_absent_entries_are_zero_and_singular_block_is_identity():
+    from workloads import CSR
+
+    # rows 0..3: only part of the block is stored; rows 4..7: a singular block (two equal rows)
+    Ad = np.zeros((8, 8))
+    Ad[0, 0], Ad[0, 2], Ad[1, 1], Ad[2, 0], Ad[2, 2], Ad[3, 3], Ad[1, 6] = 2.0, 1.0, 4.0, 1.0, 3.0, 5.0, 9.0
+    Ad[4, 4:8] = [1.0, 2.0, 3.0, 4.0]
+    Ad[5, 4:8] = [1.0, 2.0, 3.0, 4.0]
+    Ad[6, 6], Ad[7, 7] = 1.0, 1.0
+    inv = oracle.block_jacobi4(_csr_from_dense(Ad))
+    assert np.allclose(inv[0], np.linalg.inv(Ad[:4, :4]), rtol=1e-14)
+    assert np.array_equal(inv[1], np.eye(4))
+
+
+@pytest.mark.parametrize("n,seed", [(24, 90), (41, 91)])
+def test_block_jacobi4_tiny_dense_matches_direct_solve(n, seed):
+    A, Ad, b = _block_system(n, seed)
+    x0 = np.random.default_rng(seed + 2).standard_normal(n)
+    r = oracle.gmres(A, b, x0, restart=n, rel_tol=1e-11, max_iters=4 * n, fmt="fp64", precond="block_jacobi4")
+    xs = np.linalg.solve(Ad, b)
+    assert r.converged and r.iters <= n and r.restarts == 1  # the Krylov space of dimension n is the whole space
+    assert np.linalg.norm(r.x - xs) <= 1e-8 * np.linalg.norm(xs)
+    assert np.linalg.norm(b - Ad @ r.x) <= 1e-11 * np.linalg.norm(b) * (1 + 1e-6)  # residual of the ORIGINAL system
+
+
+def test_block_jacobi4_equals_plain_gmres_on_the_explicit_product():
+    """Right preconditioning is GMRES on A M^-1 in u = M x with the same residuals: the history of the
+    preconditioned run on A equals the plain run on the explicitly formed A M^-1 (numpy, input
+    construction), and x = M^-1 u.  Left / missing / transposed-block / l.17-without-M^-1 variants fail."""
+    n = 42  # ragged last block (2 rows)
+    A, Ad, b = _block_system(n, 92, coupling=0.08)
+    M = np.zeros((n, n))
+    for b0 in range(0, n, 4):
+        b1 = min(n, b0 + 4)
+        M[b0:b1, b0:b1] = Ad[b0:b1, b0:b1]
+    Minv = np.linalg.inv(M)
+    Ahat = _csr_from_dense(Ad @ Minv)
+    kw = dict(restart=5, rel_tol=1e-11, max_iters=600, fmt="fp64")
+    rp = oracle.gmres(A, b, np.zeros(n), precond="block_jacobi4", **kw)
+    ru = oracle.gmres(Ahat, b, np.zeros(n), precond="none", **kw)
+    assert rp.converged and ru.converged and rp.restarts > 2
+    assert rp.iters == ru.iters
+    live = ru.rec_history > 1e-9
+    assert np.allclose(rp.rec_history[live], ru.rec_history[live], rtol=1e-6)
+    assert np.linalg.norm(rp.x - Minv @ ru.x) <= 1e-9 * np.linalg.norm(rp.x)
+    # the transposed blocks are a different (here: much worse) preconditioner -- and so is none at all
+    AhatT = _csr_from_dense(Ad @ Minv.T)
+    rt = oracle.gmres(AhatT, b, np.zeros(n), precond="none", **kw)
+    assert (not rt.converged) or rt.iters != rp.iters
+    r0 = oracle.gmres(A, b, np.zeros(n), precond="none", **kw)
+    assert (not r0.converged) or r0.iters > rp.iters
+
+
+@pytest.mark.parametrize("fmt", ["fp64", "int16"])
+def test_block_jacobi4_reduces_to_scalar_jacobi_without_in_block_coupling(fmt):
+    """If no off-diagonal entry falls inside a 4 x 4 diagonal block, M is diag(A): same iteration as
+    the scalar preconditioner up to rounding (1/d * v against v / d)."""
+    n = 64
+    rng = np.random.default_rng(93)
+    G = 0.05 * rng.standard_normal((n, n))
+    for b0 in range(0, n, 4):
+        G[b0:b0 + 4, b0:b0 + 4] = 0.0
+    Ad = (np.eye(n) + G) * (10.0 ** rng.uniform(-1.0, 2.0, n) * rng.choice([-1.0, 1.0], n))[None, :]  # column scaling
+    A, b = _csr_from_dense(Ad), rng.standard_normal(n)
+    kw = dict(restart=8, rel_tol=1e-9, max_iters=4000, fmt=fmt)
+    s = oracle.gmres(A, b, np.zeros(n), precond="jacobi", **kw)
+    q = oracle.gmres(A, b, np.zeros(n), precond="block_jacobi4", **kw)
+    assert s.converged and q.converged
+    if fmt == "fp64":
+        assert s.iters == q.iters
+        live = s.rec_history > 1e-7
+        assert np.allclose(s.rec_history[live], q.rec_history[live], rtol=1e-6)
+    else:
+        assert abs(s.iters - q.iters) <= max(2, 0.05 * s.iters)
+    inv = oracle.block_jacobi4(A)
+    assert np.allclose(inv.reshape(-1, 4, 4)[:, np.arange(4), np.arange(4)].ravel(), 1.0 / np.diag(Ad), rtol=1e-15)
+
+
+def test_block_jacobi4_beats_scalar_jacobi_on_block_structured_matrix():
+    """What section 6.5 uses it for: on a matrix with strong 4 x 4 blocks the block preconditioner needs
+    fewer iterations than the scalar one."""
+    A, Ad, b = _block_system(200, 94, coupling=0.03)
+    kw = dict(restart=30, rel_tol=1e-9, max_iters=3000, fmt="fp64")
+    q = oracle.gmres(A, b, np.zeros(200), precond="block_jacobi4", **kw)
+    s = oracle.gmres(A, b, np.zeros(200), precond="jacobi", **kw)
+    assert q.converged and ((not s.converged) or s.iters > 2 * q.iters)
+
+
+# ---- Fig. 1 l.12: the second Gram-Schmidt pass again lost more than eta (reading Q4) -------------------------
+
+def invariant_subspace_problem(n=40, d=6, seed=95):
+    """A = blockdiag(A1, I): b lives in the first d coordinates, so the Krylov space closes at dimension
+    d: A v_d lies in span(V_d).  With a QUANTISED basis V^ the first pass leaves w1 = -V^ E c (E = V^T V^ - I,
+    about the format's unit roundoff), which triggers l.7, and the second pass leaves about E^2 c: it again
+    loses far more than eta while h_{d+1,d} stays nonzero -- only the clause `hn < eta * omega1` of l.12
+    ends the cycle there.  Hand computation: x* = [A1^-1 b1; 0]."""
+    rng = np.random.default_rng(seed)
+    A1 = rng.standard_normal((d, d)) + d * np.eye(d)
+    Ad = np.eye(n)
+    Ad[:d, :d] = A1
+    b = np.zeros(n)
+    b[:d] = rng.standard_normal(d)
+    xs = np.zeros(n)
+    xs[:d] = np.linalg.solve(A1, b[:d])
+    return _csr_from_dense(Ad), Ad, b, xs
+
+
+@pytest.mark.parametrize("fmt,u", [("fp64", 2.0 ** -53), ("fp32", 2.0 ** -24), ("fp16", 2.0 ** -11), ("int32", 2.0 ** -31),
+                                   ("int16", 2.0 ** -15)])
+def test_second_pass_breakdown_clause_ends_the_cycle(fmt, u):
+    n, d, m = 40, 6, 20
+    A, Ad, b, xs = invariant_subspace_problem(n, d)
+    # tau = 0 is out of reach, so the recurrence-residual test cannot end the cycle: only l.12 can.
+    # One cycle only (the iteration bound is met at the next restart).
+    r = oracle.gmres(A, b, np.zeros(n), restart=m, rel_tol=0.0, max_iters=d, fmt=fmt, capture_cycle=0)
+    cap = r.capture
+    H = cap["Hbar"]
+    assert cap["k"] == d and r.iters == d and r.restarts == 1
+    assert r.breakdown == 1 and not r.converged
+    # it is the eta clause, not hn == 0: h_{d+1,d} is nonzero (about omega * u^2) and far below eta * omega1
+    hn = H[d, d - 1]
+    assert 0.0 < hn < 1e-3 * cap["omega"][d - 1]
+    assert cap["reorth_log"][d - 1] == 1
+    assert r.rel_res_recurrence > 0.0
+    # no earlier step broke down although every one re-orthogonalised: there the second pass kept the norm
+    assert np.all(cap["reorth_log"] == 1) and np.all(np.diag(H, -1)[: d - 1] > 1e-2)
+    # x of that cycle against the hand computation: the minimiser over span(V^_d) = the first d coordinates,
+    # accurate to the storage format's roundoff
+    assert np.linalg.norm(r.x - xs) <= 50 * u * np.linalg.norm(xs)
+    assert not r.x[d:].any()
+    # with a reachable tau the solver restarts from the explicit residual and converges (PAPER.md:253); every
+    # cycle is cut at (or before) step d -- without the clause the first one would run on to m = 20
+    full = oracle.gmres(A, b, np.zeros(n), restart=m, rel_tol=1e-12, max_iters=200, fmt=fmt)
+    assert full.converged and np.linalg.norm(full.x - xs) <= 1e-10 * np.linalg.norm(xs)
+    assert full.iters <= d * full.restarts and full.iters <= 6 * d
+
+
+def test_second_pass_breakdown_needs_the_clause():
+    """The same problem with REORTH_NEVER has no l.12 clause (breakdown is hn == 0 only): the cycle then runs past
+    step d with a basis vector made of rounding noise -- the behaviour the clause exists to prevent."""
+    n, d, m = 40, 6, 20
+    A, Ad, b, xs = invariant_subspace_problem(n, d)
+    r = oracle.gmres(A, b, np.zeros(n), restart=m, rel_tol=0.0, max_iters=m, fmt="fp16", reorth="never",
+                     capture_cycle=0)
+    assert r.capture["k"] == m and r.breakdown == 0
