@@ -25,7 +25,9 @@
  *     solver's control block, a few MB); cbgmres_set_matrix may allocate O(nnz/1024) ints of
  *     row-partition metadata.  cbgmres_solve allocates nothing: the basis and work vectors live in
  *     the caller's workspace.
- *   - One handle per host thread.  Basis offsets are 64-bit; CSR indices are 32-bit.
+ *   - One handle per host thread; handles share no mutable state (options, error slots and per-device
+ *     kernel attributes are per handle / per device), so several handles -- on one device or on several --
+ *     can live in one process.  Basis offsets are 64-bit; CSR indices are 32-bit.
  *   - A basis is stored vector-major: vector c occupies ld entries of the storage type starting
  *     at entry c*ld; ld >= n and ld*bytes(format) must be a multiple of 16, base 16-byte aligned.
  */
@@ -68,8 +70,13 @@ typedef enum {
 /* Right preconditioner M (Fig. 1 l.3 "w := A(M^-1 v_j)", l.17 "x_m := x_0 + M^-1(V_m y_m)").
  * JACOBI: M = diag(A), the setting of every experiment in the paper; a row without a
  * nonzero diagonal entry is left unscaled.  It costs one pass over the matrix per solve and nvals*8 +
- * n*8 more workspace bytes (cbgmres_workspace_bytes accounts for them); the Arnoldi loop is unchanged. */
-typedef enum { CBGMRES_PRECOND_NONE = 0, CBGMRES_PRECOND_JACOBI = 1 } cbgmres_precond_t;
+ * n*8 more workspace bytes (cbgmres_workspace_bytes accounts for them); the Arnoldi loop is unchanged.
+ * BLOCK_JACOBI4: M = the 4 x 4 diagonal blocks of A (rows / columns 4b .. 4b+3; the last block is completed by
+ * the identity when 4 does not divide n; a singular block is replaced by the identity), inverted once per solve
+ * in fixed (fp64) precision -- the baseline of the paper's section 6.5.  The store kernel
+ * hands z = M^-1 v to the next SpMV (l.3) and the cycle end forms x += M^-1 (V_k y) (l.17).  It costs 32 bytes
+ * per row and Arnoldi step, and ceil(n/4) * 128 more workspace bytes. */
+typedef enum { CBGMRES_PRECOND_NONE = 0, CBGMRES_PRECOND_JACOBI = 1, CBGMRES_PRECOND_BLOCK_JACOBI4 = 2 } cbgmres_precond_t;
 
 #define CBGMRES_MAX_RESTART 512
 
@@ -96,6 +103,9 @@ typedef struct {
     double rel_res_true;       /* last explicit ||b - A x|| / ||b|| */
     double b_norm;
     double solve_ms;      /* device time of the whole solve (CUDA events on the stream) */
+    double algorithmic_bytes; /* bytes the method must move through HBM for the launches that ran: per Arnoldi step
+                               * S1 + S2 + S3 (+ S3' [+ S2'] where l.7 fired) + S4, per cycle S7 + S6 (cbgmres_profile_get
+                               * lists the per-kernel figures); divided by solve_ms: the whole solve's achieved GB/s */
 } cbgmres_result;
 
 /* ---- the four calls of the problem statement ------------------------------------------------ */
@@ -142,8 +152,8 @@ const char *cbgmres_last_error(cbgmres_handle_t h);
  * programmatic stream serialisation (each parks in griddepcontrol.wait until its predecessor is done).
  * "orth_fuse": 1 (default) = fuse the first update with the second pass's multi-dot (one read of V).
  * "orth_seg_kb": 0 (default, chosen per launch), 1, 2 or 4 = KB per column segment of the
- * Gram-Schmidt passes' row tiles.  "orth_interleave": 0 (default: short segments only), 1 = one
- * contiguous row range per CTA, 2 = row tiles dealt round-robin to the CTAs (process-wide knob).
+ * Gram-Schmidt passes' row tiles.  "orth_interleave": 0 (default) or 2 = row tiles dealt round-robin to
+ * the CTAs, 1 = one contiguous row range per CTA.  Every option belongs to the handle it is set on.
  * Unknown names return CBGMRES_E_INVALID. */
 int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value);
 
@@ -195,6 +205,13 @@ int cbgmres_k_update_multidot(cbgmres_handle_t h, int32_t format, int64_t n, int
  * d_payload_col[n] <- enc(v); *d_scale <- sigma.  amax = ||w||_inf (only read by the integer formats). */
 int cbgmres_k_store(cbgmres_handle_t h, int32_t format, int64_t n, const double *d_w, double hnorm, double amax,
                     void *d_payload_col, double *d_scale, double *d_v_fp64);
+/* Block-Jacobi(4): d_inv[16 b + 4 r + c] <- (A_bb^-1)_{rc} for the 4 x 4 diagonal blocks of the
+ * registered matrix, b = 0 .. ceil(n/4)-1 (caller-owned device buffer of ceil(n/4)*16 doubles). */
+int cbgmres_k_bj4_setup(cbgmres_handle_t h, double *d_inv);
+/* S4 with the block-Jacobi(4) preconditioner: as cbgmres_k_store, but d_z_fp64[i] <- (M^-1 v)_i, the vector the
+ * next SpMV multiplies (Fig. 1 l.3), with d_inv from cbgmres_k_bj4_setup.  The payload is enc(v) as before. */
+int cbgmres_k_store_bj4(cbgmres_handle_t h, int32_t format, int64_t n, const double *d_w, double hnorm, double amax,
+                        const double *d_inv, void *d_payload_col, double *d_scale, double *d_z_fp64);
 /* S1, Fig. 1 line 3: d_w <- A d_v with the registered matrix; if d_nrm2 != NULL,
  * *d_nrm2 <- ||w||_2 (omega, line 4) from the same pass. */
 int cbgmres_k_spmv(cbgmres_handle_t h, const double *d_v, double *d_w, double *d_nrm2);

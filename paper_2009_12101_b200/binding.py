@@ -20,7 +20,7 @@ FORMATS = ("fp64", "fp32", "fp16", "int32", "int16")
 FORMAT_CODE = {f: i for i, f in enumerate(FORMATS)}
 FORMAT_BYTES = {"fp64": 8, "fp32": 4, "fp16": 2, "int32": 4, "int16": 2}
 REORTH_CODE = {"never": 0, "cond": 1, "always": 2}
-PRECOND_CODE = {"none": 0, "jacobi": 1}
+PRECOND_CODE = {"none": 0, "jacobi": 1, "block_jacobi4": 2}
 STATUS = {0: "OK", 1: "E_INVALID", 2: "E_NOMATRIX", 3: "E_WORKSPACE", 4: "E_CUDA", 5: "E_NONFINITE",
           16: "NOT_CONVERGED"}
 MAX_RESTART = 512
@@ -30,6 +30,7 @@ EXPORTS = (
     "cbgmres_workspace_bytes_host", "cbgmres_solve_host", "cbgmres_destroy", "cbgmres_last_error",
     "cbgmres_set_option", "cbgmres_launch_count", "cbgmres_k_compress", "cbgmres_k_decode", "cbgmres_k_multidot",
     "cbgmres_k_update", "cbgmres_k_update_multidot", "cbgmres_k_store", "cbgmres_k_spmv", "cbgmres_profile_get", "cbgmres_profile_reset",
+    "cbgmres_k_bj4_setup", "cbgmres_k_store_bj4",
 )
 PROF_FAMILIES = ("spmv", "multidot", "update", "store", "xupdate", "residual", "update_multidot")
 
@@ -43,7 +44,8 @@ class Params(C.Structure):
 class Result(C.Structure):
     _fields_ = [("iters", C.c_int32), ("restarts", C.c_int32), ("reorth_count", C.c_int32), ("breakdown", C.c_int32),
                 ("converged", C.c_int32), ("spmv_kernel", C.c_int32), ("rel_res_recurrence", C.c_double),
-                ("rel_res_true", C.c_double), ("b_norm", C.c_double), ("solve_ms", C.c_double)]
+                ("rel_res_true", C.c_double), ("b_norm", C.c_double), ("solve_ms", C.c_double),
+                ("algorithmic_bytes", C.c_double)]
 
 
 class CbgmresError(RuntimeError):
@@ -84,6 +86,8 @@ def load_library(path: str = LIB_PATH):
     L.cbgmres_k_update_multidot.argtypes = [vp, i32, i64, i64, i32, vp, vp, vp, vp, vp, vp, vp]
     L.cbgmres_k_store.argtypes = [vp, i32, i64, vp, dbl, dbl, vp, vp, vp]
     L.cbgmres_k_spmv.argtypes = [vp, vp, vp, vp]
+    L.cbgmres_k_bj4_setup.argtypes = [vp, vp]
+    L.cbgmres_k_store_bj4.argtypes = [vp, i32, i64, vp, dbl, dbl, vp, vp, vp, vp]
     L.cbgmres_profile_get.argtypes = [vp, i32, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i64)]
     L.cbgmres_profile_reset.argtypes = [vp]
     for name in EXPORTS:
@@ -124,6 +128,7 @@ class SolveResult:
     rel_res_true: float
     b_norm: float
     solve_ms: float
+    algorithmic_bytes: float = 0.0
     rec_history: np.ndarray | None = None
 
 
@@ -225,7 +230,7 @@ class Solver:
     def solve(self, b, x0, restart: int, rel_tol: float, max_iters: int, fmt: str = "fp64", reorth: str = "cond",
               eta: float = 0.0, history: bool = False, precond: str = "none"):
         """Returns (x device tensor, SolveResult).  x0 is not modified.  precond = "jacobi": right
-        preconditioner M = diag(A)."""
+        preconditioner M = diag(A); "block_jacobi4": M = the 4 x 4 diagonal blocks."""
         torch = _torch()
         bt = self._dev(b, torch.float64)
         xt = self._dev(x0, torch.float64).clone()
@@ -262,7 +267,7 @@ class Solver:
     def _result(rc, res, hist):
         return SolveResult(rc, res.iters, res.restarts, res.reorth_count, res.breakdown, bool(res.converged),
                            res.spmv_kernel, res.rel_res_recurrence, res.rel_res_true, res.b_norm, res.solve_ms,
-                           hist[: res.iters] if hist is not None else None)
+                           res.algorithmic_bytes, hist[: res.iters] if hist is not None else None)
 
     # -- per-kernel hooks -----------------------------------------------------------------------------
     def k_compress(self, fmt: str, v):
@@ -323,6 +328,24 @@ class Solver:
         self._check(self.lib.cbgmres_k_store(self.h, FORMAT_CODE[fmt], n, _ptr(w), float(hnorm), float(amax),
                                              _ptr(payload_col), _ptr(scale), _ptr(v_out)))
         return payload_col, scale, v_out
+
+    def k_bj4_setup(self):
+        """Inverted 4 x 4 diagonal blocks of the registered matrix, device tensor [ceil(n/4), 4, 4]."""
+        torch = _torch()
+        inv = torch.empty(((self.n + 3) // 4, 4, 4), dtype=torch.float64, device=self.device)
+        self._check(self.lib.cbgmres_k_bj4_setup(self.h, _ptr(inv)))
+        return inv
+
+    def k_store_bj4(self, fmt: str, w, hnorm: float, amax: float, inv):
+        """S4 with block-Jacobi(4): returns (payload, scale, z = M^-1 v)."""
+        torch = _torch()
+        n = w.numel()
+        payload = torch.empty(n, dtype=payload_dtype(fmt), device=self.device)
+        z = torch.empty(n, dtype=torch.float64, device=self.device)
+        scale = torch.zeros(1, dtype=torch.float64, device=self.device)
+        self._check(self.lib.cbgmres_k_store_bj4(self.h, FORMAT_CODE[fmt], n, _ptr(w), float(hnorm), float(amax),
+                                                 _ptr(inv), _ptr(payload), _ptr(scale), _ptr(z)))
+        return payload, scale, z
 
     def k_spmv(self, v, w=None, want_norm: bool = True):
         torch = _torch()

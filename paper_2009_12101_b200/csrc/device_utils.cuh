@@ -317,10 +317,12 @@ __device__ __forceinline__ void bulk_g2s_hint(void *dst_smem, const void *src, u
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
-extern int g_use_pdl; // solver.cu ("pdl" option)
-
+// Launch on stream s as a link of the step chain (programmatic stream serialisation unless the handle's
+// "pdl" option is off).  A failed launch is recorded in the handle's LaunchCtx with the kernel's name
+// (the first failure wins); the solver checks it after every enqueued step.
 template <class... KArgs, class... Args>
-inline cudaError_t launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args &&...args)
+inline cudaError_t launch_chain(const Scratch &sc, const char *name, void (*kernel)(KArgs...), dim3 grid, dim3 block,
+                                size_t smem, cudaStream_t s, Args &&...args)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid;
@@ -331,8 +333,13 @@ inline cudaError_t launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block,
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
-    cfg.numAttrs = g_use_pdl ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+    cfg.numAttrs = sc.lc->use_pdl ? 1 : 0;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+    if (e != cudaSuccess && sc.lc->launch_error == cudaSuccess) {
+        sc.lc->launch_error = e;
+        sc.lc->launch_kernel = name;
+    }
+    return e;
 }
 
 // Hand a shared-memory slot back to the producer (arrive on its "empty" mbarrier) -- but only once

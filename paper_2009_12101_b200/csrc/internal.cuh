@@ -61,11 +61,33 @@ struct CycleState {
     double *hist;   // [hist_cap] recurrence residual per Arnoldi step
 };
 
+// Per-handle launch state (host side).  Everything a launcher may change or consult lives here, not in
+// process-wide globals: two handles (two devices, two streams, two host threads) do not see each other.
+struct LaunchCtx {
+    int device = 0;
+    int use_pdl = 1;      // "pdl" option: programmatic dependent launch of the step kernels
+    int interleave = 0;   // "orth_interleave" option: 0 auto, 1 blocked row ranges, 2 interleaved row tiles
+    int orth_error = 0;   // CUresult of a failed tensor-map encode (0 = none)
+    cudaError_t launch_error = cudaSuccess; // first failed kernel launch since the last take_launch_error
+    const char *launch_kernel = "";         // ... and which kernel it was
+};
+
 struct Scratch {
     Ctl *ctl;          // device
     double *partials;  // [kMaxGrid * kLdp] multi-dot partial sums, row = CTA
     double *npart;     // [2 * kMaxGrid] sum-of-squares and max partials
+    LaunchCtx *lc;     // host: the handle's launch state (never null)
 };
+
+// True the first time it is called for (this static mask, device): function attributes
+// (cudaFuncSetAttribute, occupancy queries) are per device, not per process.
+inline bool first_use_on_device(unsigned long long &mask, int device)
+{
+    const unsigned long long bit = 1ull << (device & 63);
+    if (mask & bit) return false;
+    mask |= bit;
+    return true;
+}
 
 struct BasisView {
     const void *V;     // payload, vector-major
@@ -94,11 +116,9 @@ int launch_update(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t
 int launch_update_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t n, int k, const double *hs,
                            double *w, double *h_out, double *hs_out, int mode, int step, int seg_kb);
 bool update_multidot_fits(int format, int k, int seg_kb);
-int take_orth_error();           // CUresult of a failed tensor-map encode since the last call (0 = none)
-void set_orth_interleave(int v); // tuning knob: 0 auto, 1 blocked row ranges, 2 interleaved row tiles
 int launch_store(cudaStream_t s, const Scratch &sc, int format, int64_t n, const double *w, const double *d_hn,
                  const double *d_amax, double hn_host, double amax_host, void *payload_col, double *scale_out,
-                 double *v_out, int mode, int step, const CycleState *cyc, int *h_flag);
+                 double *v_out, int mode, int step, const CycleState *cyc, int *h_flag, const double *bj_inv = nullptr);
 int launch_decode(cudaStream_t s, int format, int64_t n, const void *payload, const double *d_scale, double *v);
 int launch_spmv(cudaStream_t s, const Scratch &sc, const CsrView &A, const double *x, const double *b, double *w,
                 int mode, int step, const CycleState *cyc, int *h_flag);
@@ -109,6 +129,11 @@ int launch_copy_scalars(cudaStream_t s, const double *src0, double *dst0, const 
 
 int launch_jacobi_setup(cudaStream_t s, const CsrView &A, double *d, double *scaled_vals); // d = diag(A), vals / d[col]
 int launch_diag_scale(cudaStream_t s, int64_t n, double *x, const double *d, int inverse);  // x *= d or x /= d
+
+// Block-Jacobi(4) right preconditioner: inv[16 b + 4 r + c] = (A_bb^-1)_{rc} of the 4 x 4 diagonal blocks
+int launch_bj4_setup(cudaStream_t s, const CsrView &A, double *inv);
+int launch_bj4_axpy(cudaStream_t s, int64_t n, const double *inv, const double *t, double *x); // x += M^-1 t (Fig. 1 l.17)
+int launch_fill_zero(cudaStream_t s, int64_t n, double *x);
 
 int launch_row_stats(cudaStream_t s, int64_t n, const int32_t *d_row_ptr, int *d_out);
 

@@ -38,19 +38,6 @@ namespace cbg {
 
 enum PassKind : int { PASS_DOT = 0, PASS_UPD = 1, PASS_UPD_DOT = 2 };
 
-#ifdef CBG_TRACE // development aid: per-CTA time stamps (ns) of the last orth launch
-__device__ unsigned long long g_trace[160][48];
-__device__ __forceinline__ unsigned long long gtime()
-{
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-#define TR(i) (g_trace[blockIdx.x][(i)] = gtime())
-#else
-#define TR(i) ((void)0)
-#endif
-
 constexpr int kColWarps = 8;                            // columns per chunk: one per warp of a row half
 constexpr int kConsumerWarps = 2 * kColWarps;           // two row halves
 constexpr int kConsumers = kConsumerWarps * 32;
@@ -573,7 +560,6 @@ template <int KIND, bool SCALED> __device__ void orth_finalize(const OrthArgs &a
             }
         }
         part[sl * kMaxRangeCols + col] = sum;
-        if (tid == 0) TR(24);
     }
     if (HAS_UPD && a.last_range) {
         nt = warp_sum(nt);
@@ -584,7 +570,6 @@ template <int KIND, bool SCALED> __device__ void orth_finalize(const OrthArgs &a
         }
     }
     __syncthreads();
-    if (tid == 0) TR(25);
     if (HAS_UPD && a.last_range && tid == 0) {
         double t = 0.0, m = 0.0;
 #pragma unroll
@@ -649,7 +634,6 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
     constexpr int R = T::R, B = T::B;
     constexpr bool HAS_UPD = KIND != PASS_DOT, HAS_DOT = KIND != PASS_UPD;
     Ctl *ctl = a.ctl;
-    if (threadIdx.x == 0) TR(0);
     const int ns = a.nstages;
 
     extern __shared__ __align__(128) unsigned char smem[];
@@ -723,11 +707,9 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
         pre = nst0 < ns ? nst0 : ns;
         const int t0 = dir ? ntiles - 1 : 0;
         for (int st = 0; st < pre; ++st) issue_stage(row_begin + (int64_t)t0 * tile_stride, st, st, a.k);
-        if (lane == 0) TR(30);
     }
     pdl_wait();
     pdl_launch_dependents();
-    if (threadIdx.x == 0) TR(1);
     // the control words this CTA needs, fetched together (each is an L2 round trip)
     const int stop_after = __ldcg(&ctl->stop_after), reorth_flag = __ldcg(&ctl->reorth_flag);
     const int dk = a.d_k ? __ldcg(a.d_k) : 0;
@@ -753,7 +735,6 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
         if (tid < kMaxRangeCols) hs_s[tid] = (tid < k) ? hs_v * (upd_rowmap<FMT, F, KIND>() ? 1.0 : T::Fm::PRE) : 0.0;
         consumer_bar();
     }
-    if (threadIdx.x == 0) TR(2);
 
     double acc[kMaxChunks];
 #pragma unroll
@@ -786,7 +767,6 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
                 ring.advance(ns);
             }
         }
-        if (lane == 0) TR(31);
     } else {
         ConsumerCtx c{full, empty, wfull, wempty, hs_s, wbuf, red, red + kColWarps * R, stages, ns, k, nst, lane, warp & 7, warp >> 3, tid};
         Ring ring;
@@ -796,9 +776,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
             const int rows = (int)min((int64_t)R, row_end - r0);
             if (rows == R) consume_tile<FMT, F, KIND, false>(c, a, r0, rows, i % kWSlots, (i / kWSlots) & 1, ring, acc, ss, am);
             else consume_tile<FMT, F, KIND, true>(c, a, r0, rows, i % kWSlots, (i / kWSlots) & 1, ring, acc, ss, am);
-            if (tid == 0 && i < 16) TR(3 + i);
         }
-        if (tid == 0) TR(20);
         // ---- CTA partials ------------------------------------------------------------------------------
         if (HAS_DOT) {
             const double tot = butterfly_rec<kMaxChunks, 16>(acc, lane);
@@ -830,11 +808,8 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
         a.npart[blockIdx.x] = t;
         a.npart[kMaxGrid + blockIdx.x] = m;
     }
-    if (threadIdx.x == 0) TR(21);
     if (!last_block_done(&ctl->tickets[0])) return;
-    if (threadIdx.x == 0) TR(22);
     orth_finalize<KIND, T::Fm::SCALED>(a, k, reinterpret_cast<double *>(smem + 4096));
-    if (threadIdx.x == 0) TR(23);
 }
 
 
@@ -1034,9 +1009,6 @@ int choose_seg_kb(int format, int kind, int k, int64_t n, int forced)
     return 0;
 }
 
-int g_interleave_opt = 0; // 0 = auto (interleave), 1 = never (one contiguous row range per CTA), 2 = always
-int g_orth_error = 0;     // CUresult of the last failed tensor-map encode (0 = none)
-
 // ---- tensor maps: the basis as a 2D array [k columns][ceil(n*B/8) 8-byte words], box = 8 columns x
 // (1 or 2 KB).  Rows beyond n*B bytes and columns beyond k are out of range: not fetched, read as zero.
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -1067,7 +1039,7 @@ struct MapKey {
 };
 
 // One cached map per column count: inside a solve the same (V, k) comes back every restart cycle.
-const CUtensorMap *basis_map(const void *V, int64_t ld, int64_t n, int bytes, int k, int inner)
+const CUtensorMap *basis_map(LaunchCtx *lc, const void *V, int64_t ld, int64_t n, int bytes, int k, int inner)
 {
     struct Entry {
         MapKey key;
@@ -1079,7 +1051,7 @@ const CUtensorMap *basis_map(const void *V, int64_t ld, int64_t n, int bytes, in
     if (e.key == key) return &e.map;
     EncodeTiledFn fn = encode_fn();
     if (!fn) {
-        g_orth_error = 999; // CUDA_ERROR_UNKNOWN: the driver has no cuTensorMapEncodeTiled
+        lc->orth_error = 999; // CUDA_ERROR_UNKNOWN: the driver has no cuTensorMapEncodeTiled
         return nullptr;
     }
     const cuuint64_t dims[2] = {(cuuint64_t)((n * bytes + 7) / 8), (cuuint64_t)k};
@@ -1090,7 +1062,7 @@ const CUtensorMap *basis_map(const void *V, int64_t ld, int64_t n, int bytes, in
                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (rc != CUDA_SUCCESS) {
-        g_orth_error = (int)rc;
+        lc->orth_error = (int)rc;
         e.key = MapKey{};
         return nullptr;
     }
@@ -1100,7 +1072,7 @@ const CUtensorMap *basis_map(const void *V, int64_t ld, int64_t n, int bytes, in
 
 // w as a 2D array [n / VEC groups][VEC doubles] with box [VEC x R / VEC] and the 32/64-byte swizzle
 // (see wswz).  Only complete groups are in range; rows beyond them read as zero.
-const CUtensorMap *w_map(const double *w, int64_t n, int vec, int R)
+const CUtensorMap *w_map(LaunchCtx *lc, const double *w, int64_t n, int vec, int R)
 {
     struct Entry {
         const double *w = nullptr;
@@ -1114,7 +1086,7 @@ const CUtensorMap *w_map(const double *w, int64_t n, int vec, int R)
         if (e.w == w && e.n == n && e.vec == vec && e.R == R) return &e.map;
     EncodeTiledFn fn = encode_fn();
     if (!fn) {
-        g_orth_error = 999;
+        lc->orth_error = 999;
         return nullptr;
     }
     Entry &e = cache[next];
@@ -1129,7 +1101,7 @@ const CUtensorMap *w_map(const double *w, int64_t n, int vec, int R)
                            CU_TENSOR_MAP_INTERLEAVE_NONE, vec == 8 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_32B,
                            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (rc != CUDA_SUCCESS) {
-        g_orth_error = (int)rc;
+        lc->orth_error = (int)rc;
         return nullptr;
     }
     e.w = w;
@@ -1139,30 +1111,28 @@ const CUtensorMap *w_map(const double *w, int64_t n, int vec, int R)
     return &e.map;
 }
 
-template <int FMT, int F, int KIND> int launch_inst(cudaStream_t s, OrthArgs &a)
+template <int FMT, int F, int KIND> int launch_inst(cudaStream_t s, const Scratch &sc, OrthArgs &a)
 {
     using T = Tile<FMT, F>;
-    a.interleave = g_interleave_opt != 1; // measured: the shared sliding window wins for every segment size (fp64 k = 100: 6.46 -> 6.75 TB/s)
-    static bool attr_set = false;
-    if (!attr_set) {
+    a.interleave = sc.lc->interleave != 1; // measured: the shared sliding window wins for every segment size (fp64 k = 100: 6.46 -> 6.75 TB/s)
+    static unsigned long long attr_set = 0; // the opt-in to 225 KB of dynamic shared memory is per device
+    if (first_use_on_device(attr_set, sc.lc->device))
         cudaFuncSetAttribute(orth_kernel<FMT, F, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, kOrthSmemBytes);
-        attr_set = true;
-    }
-    const CUtensorMap *map = basis_map(a.V, a.ld, a.n, T::B, a.k, T::BOX_INNER);
+    const CUtensorMap *map = basis_map(sc.lc, a.V, a.ld, a.n, T::B, a.k, T::BOX_INNER);
     if (!map) return 0;
-    const CUtensorMap *wm = (T::VEC == 2) ? map : w_map(a.w, a.n, T::VEC, T::R); // fp64: linear w tiles, map unused
+    const CUtensorMap *wm = (T::VEC == 2) ? map : w_map(sc.lc, a.w, a.n, T::VEC, T::R); // fp64: linear w tiles, map unused
     if (!wm) return 0;
     a.nstages = stages_for(FMT, F, KIND != PASS_DOT);
     int64_t grid = (a.n + 63) / 64;
     if (grid > kNumSMs) grid = kNumSMs;
     const size_t smem = (size_t)orth_fixed_smem(T::R, KIND != PASS_DOT) + (size_t)a.nstages * T::STAGE;
-    launch_chain(orth_kernel<FMT, F, KIND>, dim3((unsigned)grid), dim3(kOrthThreads), smem, s, a, *map, *wm);
+    launch_chain(sc, "orth_kernel", orth_kernel<FMT, F, KIND>, dim3((unsigned)grid), dim3(kOrthThreads), smem, s, a, *map, *wm);
     return 1;
 }
 
 constexpr int kSmallSmemBytes = 17 * 1024; // the final stage's scratch ([16][128] doubles)
 
-template <int KIND> int launch_small(cudaStream_t s, int format, OrthArgs &a)
+template <int KIND> int launch_small(cudaStream_t s, const Scratch &sc, int format, OrthArgs &a)
 {
     const int64_t groups = a.n / (16 / fmt_bytes(format));
     int64_t grid = (groups + kOrthThreads - 1) / kOrthThreads;
@@ -1170,11 +1140,11 @@ template <int KIND> int launch_small(cudaStream_t s, int format, OrthArgs &a)
     if (grid < 1) grid = 1;
     const dim3 g((unsigned)grid), b(kOrthThreads);
     switch (format) {
-    case CBGMRES_FP64: launch_chain(orth_small_kernel<CBGMRES_FP64, KIND>, g, b, kSmallSmemBytes, s, a); break;
-    case CBGMRES_FP32: launch_chain(orth_small_kernel<CBGMRES_FP32, KIND>, g, b, kSmallSmemBytes, s, a); break;
-    case CBGMRES_FP16: launch_chain(orth_small_kernel<CBGMRES_FP16, KIND>, g, b, kSmallSmemBytes, s, a); break;
-    case CBGMRES_INT32: launch_chain(orth_small_kernel<CBGMRES_INT32, KIND>, g, b, kSmallSmemBytes, s, a); break;
-    case CBGMRES_INT16: launch_chain(orth_small_kernel<CBGMRES_INT16, KIND>, g, b, kSmallSmemBytes, s, a); break;
+    case CBGMRES_FP64: launch_chain(sc, "orth_small_kernel", orth_small_kernel<CBGMRES_FP64, KIND>, g, b, kSmallSmemBytes, s, a); break;
+    case CBGMRES_FP32: launch_chain(sc, "orth_small_kernel", orth_small_kernel<CBGMRES_FP32, KIND>, g, b, kSmallSmemBytes, s, a); break;
+    case CBGMRES_FP16: launch_chain(sc, "orth_small_kernel", orth_small_kernel<CBGMRES_FP16, KIND>, g, b, kSmallSmemBytes, s, a); break;
+    case CBGMRES_INT32: launch_chain(sc, "orth_small_kernel", orth_small_kernel<CBGMRES_INT32, KIND>, g, b, kSmallSmemBytes, s, a); break;
+    case CBGMRES_INT16: launch_chain(sc, "orth_small_kernel", orth_small_kernel<CBGMRES_INT16, KIND>, g, b, kSmallSmemBytes, s, a); break;
     default: return 0;
     }
     return 1;
@@ -1186,27 +1156,27 @@ inline bool use_small(const OrthArgs &a, int format, int forced_seg_kb)
            reinterpret_cast<uintptr_t>(a.V) % 16 == 0 && reinterpret_cast<uintptr_t>(a.w) % 16 == 0;
 }
 
-template <int FMT, int KIND> int launch_f(cudaStream_t s, OrthArgs &a, int seg_kb)
+template <int FMT, int KIND> int launch_f(cudaStream_t s, const Scratch &sc, OrthArgs &a, int seg_kb)
 {
     constexpr int VEC = Fmt<FMT>::VEC;
     switch (seg_kb) {
-    case 1: return launch_inst<FMT, 1, KIND>(s, a);
-    case 2: return launch_inst<FMT, 2, KIND>(s, a);
+    case 1: return launch_inst<FMT, 1, KIND>(s, sc, a);
+    case 2: return launch_inst<FMT, 2, KIND>(s, sc, a);
     case 4:
-        if constexpr (VEC <= 4) return launch_inst<FMT, 4, KIND>(s, a);
+        if constexpr (VEC <= 4) return launch_inst<FMT, 4, KIND>(s, sc, a);
         return 0;
     default: return 0;
     }
 }
 
-template <int KIND> int launch_fmt(cudaStream_t s, int format, OrthArgs &a, int seg_kb)
+template <int KIND> int launch_fmt(cudaStream_t s, const Scratch &sc, int format, OrthArgs &a, int seg_kb)
 {
     switch (format) {
-    case CBGMRES_FP64: return launch_f<CBGMRES_FP64, KIND>(s, a, seg_kb);
-    case CBGMRES_FP32: return launch_f<CBGMRES_FP32, KIND>(s, a, seg_kb);
-    case CBGMRES_FP16: return launch_f<CBGMRES_FP16, KIND>(s, a, seg_kb);
-    case CBGMRES_INT32: return launch_f<CBGMRES_INT32, KIND>(s, a, seg_kb);
-    case CBGMRES_INT16: return launch_f<CBGMRES_INT16, KIND>(s, a, seg_kb);
+    case CBGMRES_FP64: return launch_f<CBGMRES_FP64, KIND>(s, sc, a, seg_kb);
+    case CBGMRES_FP32: return launch_f<CBGMRES_FP32, KIND>(s, sc, a, seg_kb);
+    case CBGMRES_FP16: return launch_f<CBGMRES_FP16, KIND>(s, sc, a, seg_kb);
+    case CBGMRES_INT32: return launch_f<CBGMRES_INT32, KIND>(s, sc, a, seg_kb);
+    case CBGMRES_INT16: return launch_f<CBGMRES_INT16, KIND>(s, sc, a, seg_kb);
     default: return 0;
     }
 }
@@ -1229,24 +1199,6 @@ OrthArgs base_args(const Scratch &sc, const BasisView &b, int64_t n, int mode, i
 
 } // namespace
 
-void set_orth_interleave(int v) { g_interleave_opt = v; }
-#ifdef CBG_TRACE
-extern "C" int cbgmres_debug_trace(unsigned long long *host_out)
-{
-    return (int)cudaMemcpyFromSymbol(host_out, g_trace, sizeof(g_trace));
-}
-extern "C" int cbgmres_debug_trace_clear()
-{
-    static unsigned long long z[160][48];
-    return (int)cudaMemcpyToSymbol(g_trace, z, sizeof(z));
-}
-#endif
-int take_orth_error()
-{
-    const int e = g_orth_error;
-    g_orth_error = 0;
-    return e;
-}
 
 // S2 (and S2' when the fused pass does not fit): ranges of at most 128 columns per launch.
 int launch_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t n, int k, const double *w,
@@ -1265,8 +1217,8 @@ int launch_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b, int64
         a.h_out = h_out + c0;
         a.hs_out = hs_out ? hs_out + c0 : nullptr;
         a.last_range = (c0 + kMaxRangeCols >= k);
-        if (use_small(a, b.format, seg_kb)) launches += launch_small<PASS_DOT>(s, b.format, a);
-        else launches += launch_fmt<PASS_DOT>(s, b.format, a, choose_seg_kb(b.format, PASS_DOT, kk, n, seg_kb));
+        if (use_small(a, b.format, seg_kb)) launches += launch_small<PASS_DOT>(s, sc, b.format, a);
+        else launches += launch_fmt<PASS_DOT>(s, sc, b.format, a, choose_seg_kb(b.format, PASS_DOT, kk, n, seg_kb));
     }
     return launches;
 }
@@ -1288,8 +1240,8 @@ int launch_update(cudaStream_t s, const Scratch &sc, const BasisView &b, int64_t
         a.w = w;
         a.k = kk;
         a.last_range = (c0 + kMaxRangeCols >= k);
-        if (use_small(a, b.format, seg_kb)) launches += launch_small<PASS_UPD>(s, b.format, a);
-        else launches += launch_fmt<PASS_UPD>(s, b.format, a, choose_seg_kb(b.format, PASS_UPD, kk, n, seg_kb));
+        if (use_small(a, b.format, seg_kb)) launches += launch_small<PASS_UPD>(s, sc, b.format, a);
+        else launches += launch_fmt<PASS_UPD>(s, sc, b.format, a, choose_seg_kb(b.format, PASS_UPD, kk, n, seg_kb));
     }
     return launches;
 }
@@ -1310,8 +1262,8 @@ int launch_update_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b
     a.k = k;
     a.h_out = h_out;
     a.hs_out = hs_out;
-    if (use_small(a, b.format, seg_kb)) return launch_small<PASS_UPD_DOT>(s, b.format, a);
-    return launch_fmt<PASS_UPD_DOT>(s, b.format, a, choose_seg_kb(b.format, PASS_UPD_DOT, k, n, seg_kb));
+    if (use_small(a, b.format, seg_kb)) return launch_small<PASS_UPD_DOT>(s, sc, b.format, a);
+    return launch_fmt<PASS_UPD_DOT>(s, sc, b.format, a, choose_seg_kb(b.format, PASS_UPD_DOT, k, n, seg_kb));
 }
 
 } // namespace cbg

@@ -18,7 +18,7 @@ template <bool SCALED> __global__ void __launch_bounds__(kBackThreads) backsolve
     pdl_wait();
     pdl_launch_dependents();
     const int k = ctl->k;
-    if (k <= 0) return;
+    if (k <= 0 || ctl->nonfinite) return; // a non-finite norm: x stays at the last completed cycle (cbgmres.h)
     __shared__ double t[kMaxRestart + 1];
     __shared__ double Rs[kBackStage * (kBackStage + 1) / 2]; // column i at offset i (i + 1) / 2, rows 0..i
     const int tid = threadIdx.x, lane = tid & 31, m = ctl->m;
@@ -50,8 +50,8 @@ template <bool SCALED> __global__ void __launch_bounds__(kBackThreads) backsolve
 
 int launch_backsolve(cudaStream_t s, const Scratch &sc, const CycleState &cyc, int format)
 {
-    if (format == CBGMRES_INT32 || format == CBGMRES_INT16) launch_chain(backsolve_kernel<true>, dim3(1), dim3(kBackThreads), 0, s, sc.ctl, cyc);
-    else launch_chain(backsolve_kernel<false>, dim3(1), dim3(kBackThreads), 0, s, sc.ctl, cyc);
+    if (format == CBGMRES_INT32 || format == CBGMRES_INT16) launch_chain(sc, "backsolve_kernel", backsolve_kernel<true>, dim3(1), dim3(kBackThreads), 0, s, sc.ctl, cyc);
+    else launch_chain(sc, "backsolve_kernel", backsolve_kernel<false>, dim3(1), dim3(kBackThreads), 0, s, sc.ctl, cyc);
     return 1;
 }
 
@@ -120,6 +120,130 @@ int launch_jacobi_setup(cudaStream_t s, const CsrView &A, double *d, double *sca
 int launch_diag_scale(cudaStream_t s, int64_t n, double *x, const double *d, int inverse)
 {
     diag_scale_kernel<<<kNumSMs * 8, 256, 0, s>>>(n, x, d, inverse);
+    return 1;
+}
+
+// ---- block-Jacobi right preconditioner, block size 4 (section 6.5) -------------------------
+// M = blockdiag(A_bb), A_bb = rows and columns 4b .. 4b+3 of A (absent entries are zero; the last block is
+// completed by the identity when 4 does not divide n).  One thread gathers one block from its four CSR
+// rows and inverts it by Gauss-Jordan elimination with partial pivoting; a singular block is replaced by
+// the identity (as the scalar variant leaves a row with a zero diagonal unscaled).  Once per solve.
+// In the loop, M^-1 is applied by the store kernel (store.cu: the next SpMV multiplies z = M^-1 v, Fig. 1
+// l.3); at the end of a cycle x += M^-1 (V_k y) (l.17) by bj4_axpy_kernel below.
+__global__ void __launch_bounds__(128) bj4_setup_kernel(int64_t n, const int32_t *__restrict__ rp, const int32_t *__restrict__ ci,
+                                                        const double *__restrict__ va, double *__restrict__ inv)
+{
+    const int64_t nb = (n + 3) / 4;
+    for (int64_t b = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; b < nb; b += (int64_t)gridDim.x * blockDim.x) {
+        double a[4][8];
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int c = 0; c < 8; ++c) a[r][c] = (c == r + 4) ? 1.0 : 0.0;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int64_t i = 4 * b + r;
+            if (i >= n) {
+                a[r][r] = 1.0;
+                continue;
+            }
+            for (int32_t p = rp[i]; p < rp[i + 1]; ++p) {
+                const int64_t c = (int64_t)ci[p] - 4 * b;
+                if (c >= 0 && c < 4) {
+#pragma unroll
+                    for (int cc = 0; cc < 4; ++cc) // static register indexing
+                        if (cc == c) a[r][cc] += va[p];
+                }
+            }
+        }
+        bool singular = false;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (singular) continue;
+            int piv = k;
+            double best = fabs(a[k][k]);
+#pragma unroll
+            for (int r = k + 1; r < 4; ++r)
+                if (fabs(a[r][k]) > best) {
+                    best = fabs(a[r][k]);
+                    piv = r;
+                }
+            if (best == 0.0 || !isfinite(best)) {
+                singular = true;
+                continue;
+            }
+#pragma unroll
+            for (int r = k + 1; r < 4; ++r)
+                if (r == piv) {
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        const double t = a[k][c];
+                        a[k][c] = a[r][c];
+                        a[r][c] = t;
+                    }
+                }
+            const double d = a[k][k];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) a[k][c] = a[k][c] / d;
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                if (r == k) continue;
+                const double f = a[r][k];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) a[r][c] = fma(-f, a[k][c], a[r][c]);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) inv[16 * b + 4 * r + c] = singular ? (r == c ? 1.0 : 0.0) : a[r][c + 4];
+    }
+}
+
+// x_b += A_bb^-1 t_b, one block per thread (Fig. 1 l.17 with M = blockdiag: x := x + M^-1 (V_k y), t = V_k y)
+__global__ void __launch_bounds__(256) bj4_axpy_kernel(int64_t n, const double *__restrict__ inv, const double *__restrict__ t, double *__restrict__ x)
+{
+    const int64_t nb = (n + 3) / 4;
+    for (int64_t b = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; b < nb; b += (int64_t)gridDim.x * blockDim.x) {
+        double tv[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) tv[c] = (4 * b + c < n) ? t[4 * b + c] : 0.0;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            if (4 * b + r >= n) break;
+            const double *iv = inv + 16 * b + 4 * r;
+            const double z = fma(iv[3], tv[3], fma(iv[2], tv[2], fma(iv[1], tv[1], iv[0] * tv[0])));
+            x[4 * b + r] += z;
+        }
+    }
+}
+
+__global__ void fill_zero_kernel(int64_t n, double *__restrict__ x)
+{
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) x[i] = 0.0;
+}
+
+int launch_bj4_setup(cudaStream_t s, const CsrView &A, double *inv)
+{
+    const int64_t nb = (A.n + 3) / 4;
+    int64_t grid = (nb + 127) / 128;
+    if (grid > kNumSMs * 16) grid = kNumSMs * 16;
+    bj4_setup_kernel<<<(int)grid, 128, 0, s>>>(A.n, A.row_ptr, A.col_idx, A.vals, inv);
+    return 1;
+}
+
+int launch_bj4_axpy(cudaStream_t s, int64_t n, const double *inv, const double *t, double *x)
+{
+    const int64_t nb = (n + 3) / 4;
+    int64_t grid = (nb + 255) / 256;
+    if (grid > kNumSMs * 8) grid = kNumSMs * 8;
+    bj4_axpy_kernel<<<(int)grid, 256, 0, s>>>(n, inv, t, x);
+    return 1;
+}
+
+int launch_fill_zero(cudaStream_t s, int64_t n, double *x)
+{
+    fill_zero_kernel<<<kNumSMs * 8, 256, 0, s>>>(n, x);
     return 1;
 }
 

@@ -17,10 +17,6 @@
 
 using namespace cbg;
 
-namespace cbg {
-int g_use_pdl = 1; // programmatic dependent launch of the step kernels ("pdl" option)
-}
-
 struct ProfSlot {
     cudaEvent_t a = nullptr, b = nullptr;
     int family = 0, step = 0, pass = 0;
@@ -34,6 +30,7 @@ struct ProfAcc {
 struct cbgmres_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
+    LaunchCtx lc{};            // per-handle launch options and error slots (no process-wide state)
     Scratch sc{};
     void *scratch_base = nullptr;
     double *hook_hs = nullptr; // [kMaxRestart] coefficients of the k_update hook
@@ -100,6 +97,7 @@ struct Layout {
     size_t off_V, off_v, off_w, off_small, total;
     size_t o_h, o_hs, o_R, o_cs, o_sn, o_g, o_y, o_scales, o_hist;
     size_t off_pvals, off_pdiag; // Jacobi: column-scaled values and diag(A) (unused otherwise)
+    size_t off_bjinv;            // block-Jacobi(4): the inverted diagonal blocks, 16 doubles per block
 };
 
 Layout make_layout(int64_t n, int64_t nnz, const cbgmres_params *p)
@@ -120,6 +118,10 @@ Layout make_layout(int64_t n, int64_t nnz, const cbgmres_params *p)
         o += up256((size_t)nnz * 8);
         L.off_pdiag = o;
         o += up256((size_t)n * 8);
+    }
+    if (p->precond == CBGMRES_PRECOND_BLOCK_JACOBI4) {
+        L.off_bjinv = o;
+        o += up256((size_t)((n + 3) / 4) * 16 * 8);
     }
     L.off_small = o;
     size_t s = 0;
@@ -151,7 +153,8 @@ int validate_params(cbgmres_ctx *h, const cbgmres_params *p)
     if (!(p->rel_tol >= 0.0)) return fail(h, CBGMRES_E_INVALID, "rel_tol must be >= 0");
     if (!(p->eta >= 0.0) || p->eta > 1.0) return fail(h, CBGMRES_E_INVALID, "eta must be in [0, 1]");
     if (p->res_history_cap < 0) return fail(h, CBGMRES_E_INVALID, "res_history_cap < 0");
-    if (p->precond != CBGMRES_PRECOND_NONE && p->precond != CBGMRES_PRECOND_JACOBI)
+    if (p->precond != CBGMRES_PRECOND_NONE && p->precond != CBGMRES_PRECOND_JACOBI &&
+        p->precond != CBGMRES_PRECOND_BLOCK_JACOBI4)
         return fail(h, CBGMRES_E_INVALID, "unknown preconditioner");
     return CBGMRES_OK;
 }
@@ -198,6 +201,25 @@ void prof_collect(cbgmres_ctx *h, const Ctl &c, bool cycle_ran)
         acc.launches += 1;
     }
     h->prof_used = 0;
+}
+
+// A failed kernel launch or tensor-map encode recorded by a launcher since the last call (0 = none).
+int take_launch_errors(cbgmres_ctx *h)
+{
+    LaunchCtx &lc = h->lc;
+    int rc = CBGMRES_OK;
+    if (lc.launch_error != cudaSuccess) {
+        snprintf(h->err, sizeof(h->err), "launch of %s failed: %s", lc.launch_kernel, cudaGetErrorString(lc.launch_error));
+        (void)cudaGetLastError(); // clear the sticky-less launch error so that later calls start clean
+        rc = CBGMRES_E_CUDA;
+    } else if (lc.orth_error) {
+        snprintf(h->err, sizeof(h->err), "cuTensorMapEncodeTiled failed for the basis (CUresult %d)", lc.orth_error);
+        rc = CBGMRES_E_CUDA;
+    }
+    lc.launch_error = cudaSuccess;
+    lc.launch_kernel = "";
+    lc.orth_error = 0;
+    return rc;
 }
 
 int choose_spmv_kernel(cbgmres_ctx *h, int64_t n, int64_t nnz, int max_len)
@@ -261,6 +283,8 @@ int cbgmres_create(cbgmres_handle_t *out, int device, void *cuda_stream)
     cbgmres_ctx *h = new (std::nothrow) cbgmres_ctx();
     if (!h) return CBGMRES_E_INVALID;
     h->device = device;
+    h->lc.device = device;
+    h->sc.lc = &h->lc;
     h->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     cudaError_t e = cudaSetDevice(device);
     if (e != cudaSuccess) {
@@ -342,7 +366,7 @@ int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value)
     }
     if (!strcmp(name, "orth_interleave")) {
         if (value < 0 || value > 2) return fail(h, CBGMRES_E_INVALID, "orth_interleave must be 0, 1 or 2");
-        set_orth_interleave((int)value);
+        h->lc.interleave = (int)value;
         return CBGMRES_OK;
     }
     if (!strcmp(name, "orth_fuse")) {
@@ -350,7 +374,7 @@ int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value)
         return CBGMRES_OK;
     }
     if (!strcmp(name, "pdl")) {
-        g_use_pdl = value != 0;
+        h->lc.use_pdl = value != 0;
         return CBGMRES_OK;
     }
     if (!strcmp(name, "profile")) {
@@ -451,10 +475,13 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
     }
     if (!std::isfinite(bnorm)) return fail(h, CBGMRES_E_NONFINITE, "||b|| is not finite");
 
-    // Scalar Jacobi: GMRES on A D^-1 in u = D x (small.cu); d_x holds u until the end
+    // Scalar Jacobi: GMRES on A D^-1 in u = D x (small.cu); d_x holds u until the end.
+    // Block-Jacobi(4): the store kernel hands z = M^-1 v to the SpMV (l.3) and the cycle end
+    // forms x += M^-1 (V_k y) (l.17); x stays in the original variable.
     const bool jacobi = p->precond == CBGMRES_PRECOND_JACOBI;
+    const bool bj4 = p->precond == CBGMRES_PRECOND_BLOCK_JACOBI4;
     CsrView A = h->A;
-    double *pdiag = nullptr;
+    double *pdiag = nullptr, *bjinv = nullptr;
     if (jacobi) {
         double *pvals = reinterpret_cast<double *>(ws + L.off_pvals);
         pdiag = reinterpret_cast<double *>(ws + L.off_pdiag);
@@ -462,11 +489,19 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
         h->launches += launch_diag_scale(s, n, d_x, pdiag, 0);
         A.vals = pvals;
     }
+    if (bj4) {
+        bjinv = reinterpret_cast<double *>(ws + L.off_bjinv);
+        h->launches += launch_bj4_setup(s, h->A, bjinv);
+    }
     volatile int *flag = h->h_flag;
     const double dn = (double)n, dB = (double)B;
     const double bytes_spmv = 12.0 * (double)h->A.nnz + 4.0 * (dn + 1.0) + 16.0 * dn;
-    const double bytes_store = (16.0 + dB) * dn;
+    const double bytes_store = (16.0 + dB) * dn + (bj4 ? 32.0 * dn : 0.0);
     const int sk = h->opt_seg_kb;
+    double alg_bytes = 0.0;
+    // The restart cycles.  Any failure leaves through `return`; the caller below undoes the Jacobi change of
+    // variable on EVERY exit, so d_x never stays in the variable u = D x.
+    auto cycles = [&]() -> int {
     for (;;) {
         *flag = INT_MAX;
         h->prof_used = 0;
@@ -476,7 +511,7 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
         prof_begin(h, CBGMRES_PROF_RESIDUAL, 0, 0, bytes_spmv + 8.0 * dn + bytes_store);
         h->launches += launch_spmv(s, h->sc, A, d_x, d_b, w, MODE_RESIDUAL, 0, &cy, h->d_flag);
         h->launches += launch_store(s, h->sc, fmt, n, w, &dctl->hn, &dctl->amax, 0.0, 0.0, Vp, cy.scales, v,
-                                    MODE_RESIDUAL, 1, nullptr, nullptr);
+                                    MODE_RESIDUAL, 1, nullptr, nullptr, bjinv);
         prof_end(h);
         for (int j = 1; j <= m; ++j) {
             if (h->opt_poll && *flag < j) break; // the device already left this cycle
@@ -520,21 +555,40 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
             prof_begin(h, CBGMRES_PROF_STORE, j, 0, bytes_store);
             h->launches += launch_store(s, h->sc, fmt, n, w, &dctl->hn, &dctl->amax, 0.0, 0.0,
                                         Vp + (size_t)j * (size_t)L.ld * (size_t)B, cy.scales + j, v, MODE_ORTH1, j, &cy,
-                                        h->d_flag);
+                                        h->d_flag, bjinv);
             prof_end(h);
+            if (h->lc.launch_error != cudaSuccess || h->lc.orth_error) break; // a launch of this step failed: stop enqueueing
         }
-        // l.16-17: R y = g ; x += V_k y  (k read on the device)
+        // l.16-17: R y = g ; x += M^-1 (V_k y)  (k read on the device)
         h->prof_on = h->opt_profile != 0;
         prof_begin(h, CBGMRES_PROF_XUPDATE, 0, 0, 0.0);
         h->launches += launch_backsolve(s, h->sc, cy, fmt);
-        h->launches += launch_update(s, h->sc, bv, n, m, &dctl->k, cy.hs, d_x, MODE_XUPDATE, 0, sk);
+        if (bj4) { // t = V_k y in the (now free) work vector, then x += M^-1 t
+            h->launches += launch_fill_zero(s, n, w);
+            h->launches += launch_update(s, h->sc, bv, n, m, &dctl->k, cy.hs, w, MODE_XUPDATE, 0, sk);
+            h->launches += launch_bj4_axpy(s, n, bjinv, w, d_x);
+        } else {
+            h->launches += launch_update(s, h->sc, bv, n, m, &dctl->k, cy.hs, d_x, MODE_XUPDATE, 0, sk);
+        }
         prof_end(h);
         CK(cudaMemcpyAsync(h->h_ctl, dctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
         CK(cudaStreamSynchronize(s));
+        {
+            const int lrc = take_launch_errors(h);
+            if (lrc) return lrc;
+        }
         CK(cudaGetLastError());
-        if (take_orth_error()) {
-            if (jacobi) launch_diag_scale(s, n, d_x, pdiag, 1);
-            return fail(h, CBGMRES_E_CUDA, "cuTensorMapEncodeTiled failed for the basis");
+        if (h->h_ctl->restarts > restarts_before) { // algorithmic bytes of the launches that ran
+            const Ctl &c = *h->h_ctl;
+            double by = bytes_spmv + 8.0 * dn + bytes_store; // l.1: residual + store of v_1
+            for (int j = 1; j <= c.k; ++j) {
+                const double dot = (double)j * dn * dB + 8.0 * dn, upd = (double)j * dn * dB + 16.0 * dn;
+                const bool fused = p->reorth != CBGMRES_REORTH_NEVER && h->opt_fuse && update_multidot_fits(fmt, j, sk);
+                by += bytes_spmv + dot + upd + bytes_store;          // S1, S2, S3 (fused: S3 + S2' from one read), S4
+                if (c.reorth_log[j]) by += fused ? upd : dot + upd;  // S3' (and a separate S2' where the fusion does not fit)
+            }
+            if (c.k > 0) by += (double)c.k * dn * dB + 16.0 * dn;    // S6: x += V_k y
+            alg_bytes += by;
         }
         if (h->opt_profile) {
             const bool cycle_ran = h->h_ctl->restarts > restarts_before;
@@ -546,7 +600,14 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
         }
         if (h->h_ctl->done) break;
     }
-    if (jacobi) h->launches += launch_diag_scale(s, n, d_x, pdiag, 1); // l.17: x = M^-1 u
+    return CBGMRES_OK;
+    };
+    rc = cycles();
+    if (jacobi) { // l.17: x = M^-1 u -- on every exit, also the failed ones (x then holds the last iterate reached)
+        h->launches += launch_diag_scale(s, n, d_x, pdiag, 1);
+        if (rc != CBGMRES_OK) cudaStreamSynchronize(s);
+    }
+    if (rc != CBGMRES_OK) return rc;
     if (hist_cap) {
         const int cnt = h->h_ctl->iters < hist_cap ? h->h_ctl->iters : hist_cap;
         if (cnt > 0) CK(cudaMemcpyAsync(p->h_res_history, cy.hist, (size_t)cnt * 8, cudaMemcpyDeviceToHost, s));
@@ -564,6 +625,7 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
     out->rel_res_recurrence = c.rel_rec;
     out->rel_res_true = c.rel_true;
     out->solve_ms = ms;
+    out->algorithmic_bytes = alg_bytes;
     (void)launches0;
     if (c.nonfinite) return fail(h, CBGMRES_E_NONFINITE, "non-finite residual norm");
     return c.converged ? CBGMRES_OK : CBGMRES_NOT_CONVERGED;
@@ -638,6 +700,16 @@ int cbgmres_profile_reset(cbgmres_handle_t h)
 }
 
 // ---- per-kernel hooks -------------------------------------------------------------------------------
+// Every hook ends here: a launch that failed (recorded by launch_chain with the kernel's name), a failed
+// tensor-map encode, or any other pending CUDA error becomes this call's status.
+static int finish_hook(cbgmres_ctx *h)
+{
+    const int lrc = take_launch_errors(h);
+    if (lrc) return lrc;
+    CK(cudaGetLastError());
+    return CBGMRES_OK;
+}
+
 static int check_basis_args(cbgmres_ctx *h, int32_t format, int64_t n, int64_t ld, int32_t k, const void *V)
 {
     const int B = format_bytes(format);
@@ -661,8 +733,7 @@ int cbgmres_k_compress(cbgmres_handle_t h, int32_t format, int64_t n, const doub
     h->launches += launch_nrm2(h->stream, h->sc, n, d_v, MODE_HOOK);
     h->launches += launch_store(h->stream, h->sc, format, n, d_v, nullptr, &h->sc.ctl->hook_amax, 1.0, 0.0, d_payload,
                                 d_scale, nullptr, MODE_HOOK, 0, nullptr, nullptr);
-    CK(cudaGetLastError());
-    return CBGMRES_OK;
+    return finish_hook(h);
 }
 
 int cbgmres_k_decode(cbgmres_handle_t h, int32_t format, int64_t n, const void *d_payload, const double *d_scale,
@@ -674,8 +745,7 @@ int cbgmres_k_decode(cbgmres_handle_t h, int32_t format, int64_t n, const void *
         return fail(h, CBGMRES_E_INVALID, "fixed-point formats need d_scale");
     CK(cudaSetDevice(h->device));
     h->launches += launch_decode(h->stream, format, n, d_payload, d_scale, d_v);
-    CK(cudaGetLastError());
-    return CBGMRES_OK;
+    return finish_hook(h);
 }
 
 int cbgmres_k_multidot(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld, int32_t k, const void *d_V,
@@ -691,9 +761,7 @@ int cbgmres_k_multidot(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld
     CK(cudaSetDevice(h->device));
     BasisView bv{d_V, ld, d_scales, format};
     h->launches += launch_multidot(h->stream, h->sc, bv, n, k, d_w, d_h, nullptr, MODE_HOOK, 0, h->opt_seg_kb);
-    if (take_orth_error()) return fail(h, CBGMRES_E_CUDA, "cuTensorMapEncodeTiled failed for the basis");
-    CK(cudaGetLastError());
-    return CBGMRES_OK;
+    return finish_hook(h);
 }
 
 int cbgmres_k_update(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld, int32_t k, const void *d_V,
@@ -711,11 +779,9 @@ int cbgmres_k_update(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld, 
     BasisView bv{d_V, ld, d_scales, format};
     h->launches += launch_scale_coeffs(h->stream, k, d_h, scaled ? d_scales : nullptr, h->hook_hs);
     h->launches += launch_update(h->stream, h->sc, bv, n, k, nullptr, h->hook_hs, d_w, MODE_HOOK, 0, h->opt_seg_kb);
-    if (take_orth_error()) return fail(h, CBGMRES_E_CUDA, "cuTensorMapEncodeTiled failed for the basis");
     if (d_nrm2 || d_amax)
         h->launches += launch_copy_scalars(h->stream, &h->sc.ctl->hook_nrm2, d_nrm2, &h->sc.ctl->hook_amax, d_amax);
-    CK(cudaGetLastError());
-    return CBGMRES_OK;
+    return finish_hook(h);
 }
 
 int cbgmres_k_update_multidot(cbgmres_handle_t h, int32_t format, int64_t n, int64_t ld, int32_t k, const void *d_V,
@@ -737,11 +803,9 @@ int cbgmres_k_update_multidot(cbgmres_handle_t h, int32_t format, int64_t n, int
     h->launches += launch_scale_coeffs(h->stream, k, d_h, scaled ? d_scales : nullptr, h->hook_hs);
     h->launches += launch_update_multidot(h->stream, h->sc, bv, n, k, h->hook_hs, d_w, d_u, nullptr, MODE_HOOK, 0,
                                           h->opt_seg_kb);
-    if (take_orth_error()) return fail(h, CBGMRES_E_CUDA, "cuTensorMapEncodeTiled failed for the basis");
     if (d_nrm2 || d_amax)
         h->launches += launch_copy_scalars(h->stream, &h->sc.ctl->hook_nrm2, d_nrm2, &h->sc.ctl->hook_amax, d_amax);
-    CK(cudaGetLastError());
-    return CBGMRES_OK;
+    return finish_hook(h);
 }
 
 int cbgmres_k_store(cbgmres_handle_t h, int32_t format, int64_t n, const double *d_w, double hnorm, double amax,
@@ -756,8 +820,32 @@ int cbgmres_k_store(cbgmres_handle_t h, int32_t format, int64_t n, const double 
     CK(cudaSetDevice(h->device));
     h->launches += launch_store(h->stream, h->sc, format, n, d_w, nullptr, nullptr, hnorm, amax, d_payload_col, d_scale,
                                 d_v_fp64, MODE_HOOK, 0, nullptr, nullptr);
-    CK(cudaGetLastError());
-    return CBGMRES_OK;
+    return finish_hook(h);
+}
+
+int cbgmres_k_bj4_setup(cbgmres_handle_t h, double *d_inv)
+{
+    if (!h) return CBGMRES_E_INVALID;
+    if (!h->has_matrix) return fail(h, CBGMRES_E_NOMATRIX, "set_matrix has not been called");
+    if (!d_inv || reinterpret_cast<uintptr_t>(d_inv) % 16 != 0) return fail(h, CBGMRES_E_INVALID, "d_inv must be a 16-byte aligned device buffer");
+    CK(cudaSetDevice(h->device));
+    h->launches += launch_bj4_setup(h->stream, h->A, d_inv);
+    return finish_hook(h);
+}
+
+int cbgmres_k_store_bj4(cbgmres_handle_t h, int32_t format, int64_t n, const double *d_w, double hnorm, double amax,
+                        const double *d_inv, void *d_payload_col, double *d_scale, double *d_z_fp64)
+{
+    if (!h) return CBGMRES_E_INVALID;
+    if (format_bytes(format) < 0 || n <= 0 || !d_w || !d_payload_col || !d_scale || !d_inv || !d_z_fp64)
+        return fail(h, CBGMRES_E_INVALID, "bad argument");
+    if (reinterpret_cast<uintptr_t>(d_w) % 16 != 0 || reinterpret_cast<uintptr_t>(d_payload_col) % 16 != 0 ||
+        reinterpret_cast<uintptr_t>(d_z_fp64) % 16 != 0 || reinterpret_cast<uintptr_t>(d_inv) % 16 != 0)
+        return fail(h, CBGMRES_E_INVALID, "buffers must be 16-byte aligned");
+    CK(cudaSetDevice(h->device));
+    h->launches += launch_store(h->stream, h->sc, format, n, d_w, nullptr, nullptr, hnorm, amax, d_payload_col, d_scale,
+                                d_z_fp64, MODE_HOOK, 0, nullptr, nullptr, d_inv);
+    return finish_hook(h);
 }
 
 int cbgmres_k_spmv(cbgmres_handle_t h, const double *d_v, double *d_w, double *d_nrm2)
@@ -768,8 +856,7 @@ int cbgmres_k_spmv(cbgmres_handle_t h, const double *d_v, double *d_w, double *d
     CK(cudaSetDevice(h->device));
     h->launches += launch_spmv(h->stream, h->sc, h->A, d_v, nullptr, d_w, MODE_HOOK, 0, nullptr, nullptr);
     if (d_nrm2) h->launches += launch_copy_scalars(h->stream, &h->sc.ctl->hook_nrm2, d_nrm2, nullptr, nullptr);
-    CK(cudaGetLastError());
-    return CBGMRES_OK;
+    return finish_hook(h);
 }
 
 } // extern "C"

@@ -27,6 +27,19 @@ struct SpmvArgs {
     int *h_flag;
 };
 
+// Gather of one entry of x.  x is the fp64 v that the preceding store kernel wrote; under programmatic
+// dependent launch this grid can be resident while that kernel is still running, so x is NOT read-only
+// for this kernel's lifetime and must not go through ld.global.nc (which `const __restrict__` or __ldg
+// would select).  A plain L1-cached load issued after griddepcontrol.wait sees the predecessor's writes;
+// L1 matters for the stencils, where the diagonals of consecutive rows share lines.  Only the matrix
+// arrays, which no kernel ever writes, use the non-coherent path.
+__device__ __forceinline__ double ld_x(const double *p)
+{
+    double r;
+    asm volatile("ld.global.ca.f64 %0, [%1];" : "=d"(r) : "l"(p));
+    return r;
+}
+
 // Norm finalisation shared by all SpMV variants and the plain norm kernel: called by every thread
 // of the CTA that arrived last, with this CTA's (sum of squares, max) partial already in npart.
 __device__ __forceinline__ void finalize_norms(const SpmvArgs &a)
@@ -158,11 +171,11 @@ template <int LANES, int U> __global__ void __launch_bounds__(256) spmv_vec_kern
             more |= p[u] + LANES < p1[u];
         }
 #pragma unroll
-        for (int u = 0; u < U; ++u) s[u] = v[u] * x[c[u]];
+        for (int u = 0; u < U; ++u) s[u] = v[u] * ld_x(x + c[u]);
         if (__any_sync(0xffffffffu, more)) {
 #pragma unroll
             for (int u = 0; u < U; ++u)
-                for (int q = p[u] + LANES; q < p1[u]; q += LANES) s[u] = fma(va[q], x[ci[q]], s[u]);
+                for (int q = p[u] + LANES; q < p1[u]; q += LANES) s[u] = fma(va[q], ld_x(x + ci[q]), s[u]);
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
@@ -228,7 +241,7 @@ __device__ __forceinline__ double gather_x(const double *p)
     asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(r) : "l"(p));
     return r;
 #else
-    return __ldg(p);
+    return ld_x(p);
 #endif
 }
 
@@ -324,7 +337,7 @@ __global__ void __launch_bounds__(kStreamThreads) spmv_stream_kernel(const SpmvA
             // next to short ones): one warp per row straight from global memory
             for (int r = r0 + warp; r < r1; r += kStreamThreads / 32) {
                 double s = 0.0;
-                for (int p = rp[r] + lane; p < rp[r + 1]; p += 32) s = fma(va[p], x[ci[p]], s);
+                for (int p = rp[r] + lane; p < rp[r + 1]; p += 32) s = fma(va[p], ld_x(x + ci[p]), s);
                 s = warp_sum(s);
                 if (lane == 0) {
                     const double val = (a.mode == MODE_RESIDUAL) ? a.b[r] - s : s;
@@ -493,7 +506,7 @@ template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_
 #pragma unroll
                         for (int u = 0; u < RPT; ++u)
 #pragma unroll
-                            for (int k = 0; k < KU; ++k) xv[u][k] = __ldg(x + c[u][k]);
+                            for (int k = 0; k < KU; ++k) xv[u][k] = ld_x(x + c[u][k]);
                         more = false;
 #pragma unroll
                         for (int u = 0; u < RPT; ++u) {
@@ -523,7 +536,7 @@ template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_
 #pragma unroll
                     for (int u = 0; u < RPT; ++u)
 #pragma unroll
-                        for (int k = 0; k < KU; ++k) xv[u][k] = __ldg(x + c[u][k]);
+                        for (int k = 0; k < KU; ++k) xv[u][k] = ld_x(x + c[u][k]);
                     more = false;
 #pragma unroll
                     for (int u = 0; u < RPT; ++u) {
@@ -560,7 +573,7 @@ template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_
                 if (lane == 0) mbar_arrive(&sm.empty[ring.s]);
                 for (int r = r0 + warp; r < r1; r += kRowsThreads / 32) { // oversized block: warp per row from global
                     double t = 0.0;
-                    for (int p = rp[r] + lane; p < rp[r + 1]; p += 32) t = fma(va[p], x[ci[p]], t);
+                    for (int p = rp[r] + lane; p < rp[r + 1]; p += 32) t = fma(va[p], ld_x(x + ci[p]), t);
                     t = warp_sum(t);
                     if (lane == 0) {
                         const double val = (a.mode == MODE_RESIDUAL) ? a.b[r] - t : t;
@@ -576,17 +589,15 @@ template <int RPT, int LPR> __global__ void __launch_bounds__(kRowsCta, 2) spmv_
     block_norm_partials(a, ss, am, &a.ctl->tickets[2]);
 }
 
-template <int RPT, int LPR> static void launch_rows(cudaStream_t s, const SpmvArgs &a)
+template <int RPT, int LPR> static void launch_rows(cudaStream_t s, const Scratch &sc, const SpmvArgs &a)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static unsigned long long attr_set = 0; // per device
+    if (first_use_on_device(attr_set, sc.lc->device))
         cudaFuncSetAttribute(spmv_rows_kernel<RPT, LPR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RowsSmem));
-        attr_set = true;
-    }
     constexpr int RB = kRowsThreads * RPT / LPR;
     const int64_t nblk = (a.A.n + RB - 1) / RB;
     const int grid = (int)(nblk < 2 * kNumSMs ? nblk : 2 * kNumSMs); // persistent: two CTAs per SM
-    launch_chain(spmv_rows_kernel<RPT, LPR>, dim3(grid), dim3(kRowsCta), sizeof(RowsSmem), s, a);
+    launch_chain(sc, "spmv_rows_kernel", spmv_rows_kernel<RPT, LPR>, dim3(grid), dim3(kRowsCta), sizeof(RowsSmem), s, a);
 }
 
 // Row partition of the streaming kernel: block b = rows [R(b), R(b+1)) with R(b) the first row r with
@@ -669,14 +680,14 @@ int launch_nrm2(cudaStream_t s, const Scratch &sc, int64_t n, const double *x, i
     return 1;
 }
 
-template <int LANES> static void launch_vec(cudaStream_t s, const SpmvArgs &a)
+template <int LANES> static void launch_vec(cudaStream_t s, const Scratch &sc, const SpmvArgs &a)
 {
     constexpr int RPB = 256 / LANES, U = 4;
     int64_t grid = (a.A.n + RPB * U - 1) / (RPB * U);
     const int64_t cap = (int64_t)kNumSMs * 8;
     if (grid > cap) grid = cap;
     if (grid < 1) grid = 1;
-    launch_chain(spmv_vec_kernel<LANES, U>, dim3((unsigned)grid), dim3(256), 0, s, a);
+    launch_chain(sc, "spmv_vec_kernel", spmv_vec_kernel<LANES, U>, dim3((unsigned)grid), dim3(256), 0, s, a);
 }
 
 int launch_spmv(cudaStream_t s, const Scratch &sc, const CsrView &A, const double *x, const double *b, double *w,
@@ -695,30 +706,30 @@ int launch_spmv(cudaStream_t s, const Scratch &sc, const CsrView &A, const doubl
     a.step = step;
     a.h_flag = h_flag;
     switch (A.kernel) {
-    case 2: launch_vec<2>(s, a); break;
-    case 4: launch_vec<4>(s, a); break;
-    case 8: launch_vec<8>(s, a); break;
-    case 16: launch_vec<16>(s, a); break;
-    case 32: launch_vec<32>(s, a); break;
+    case 2: launch_vec<2>(s, sc, a); break;
+    case 4: launch_vec<4>(s, sc, a); break;
+    case 8: launch_vec<8>(s, sc, a); break;
+    case 16: launch_vec<16>(s, sc, a); break;
+    case 32: launch_vec<32>(s, sc, a); break;
     case 64: {
         static int per_sm = 0; // persistent grid: exactly the CTAs that are resident at once (one more per SM
-                               // and the stragglers run as a second wave: +25 % on C4)
+                               // and the stragglers run as a second wave: +25 % on C4); the same on every B200
         if (!per_sm) {
             if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spmv_stream_kernel, kStreamThreads, 0) != cudaSuccess || per_sm < 1)
                 per_sm = 1;
         }
         int grid = A.nblk < kNumSMs * per_sm ? A.nblk : kNumSMs * per_sm;
         if (grid < 1) grid = 1;
-        launch_chain(spmv_stream_kernel, dim3(grid), dim3(kStreamThreads), 0, s, a);
+        launch_chain(sc, "spmv_stream_kernel", spmv_stream_kernel, dim3(grid), dim3(kStreamThreads), 0, s, a);
         break;
     }
     // row-major kernel: 128 + rows per thread, or 144 + lanes per row
-    case 129: launch_rows<1, 1>(s, a); break;
-    case 130: launch_rows<2, 1>(s, a); break;
-    case 132: launch_rows<4, 1>(s, a); break;
-    case 146: launch_rows<1, 2>(s, a); break;
-    case 148: launch_rows<1, 4>(s, a); break;
-    case 152: launch_rows<1, 8>(s, a); break;
+    case 129: launch_rows<1, 1>(s, sc, a); break;
+    case 130: launch_rows<2, 1>(s, sc, a); break;
+    case 132: launch_rows<4, 1>(s, sc, a); break;
+    case 146: launch_rows<1, 2>(s, sc, a); break;
+    case 148: launch_rows<1, 4>(s, sc, a); break;
+    case 152: launch_rows<1, 8>(s, sc, a); break;
     default: return 0;
     }
     return 1;

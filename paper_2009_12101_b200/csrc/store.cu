@@ -21,6 +21,7 @@ struct StoreArgs {
     int has_cyc;
     int mode, step;
     int *h_flag;                 // mapped host word: mirrors ctl->stop_after (may be null)
+    const double *bj_inv;        // block-Jacobi(4): inverted diagonal blocks [ceil(n/4)][16]; v_out then receives M^-1 v
 };
 
 // The control CTA: apply rotations 1..j-1 to the new column, form rotation j, rotate g, decide
@@ -86,35 +87,39 @@ __device__ void givens_step(const StoreArgs &a)
     for (int c = tid; c < j; c += nt) Rcol[c] = s_h[c];
 }
 
-template <int FMT, int THREADS> __global__ void __launch_bounds__(THREADS) store_kernel(const StoreArgs a)
+// BJ: with the block-Jacobi(4) right preconditioner the vector the next SpMV multiplies is
+// z = M^-1 v (Fig. 1 l.3), so the store writes z instead of v: the thread that holds the four entries of
+// a block multiplies them by the block's inverse (a.bj_inv, 16 doubles per block, row-major) -- 32 bytes
+// more per row and no extra launch.  A thread then owns RT = max(VEC, 4) consecutive rows.
+template <int FMT, int THREADS, bool BJ> __global__ void __launch_bounds__(THREADS) store_kernel(const StoreArgs a)
 {
     using F = Fmt<FMT>;
     constexpr int VEC = F::VEC;
+    constexpr int GROUPS = (BJ && VEC < 4) ? 4 / VEC : 1; // 16-byte payload words per thread and iteration
+    constexpr int RT = VEC * GROUPS;                       // rows per thread and iteration
     pdl_wait();
     // A successor may fetch basis columns before ITS grid dependency resolves (orth.cu); inside a solve
     // the successor of a store is never a Gram-Schmidt pass, but after the k_compress / k_store hooks it
     // can be: there the successor is only released when this kernel has completed.
     if (a.mode != MODE_HOOK) pdl_launch_dependents();
     // this thread's first rows of w and the control words, fetched together (each is an L2 round trip)
-    const bool has_ctl_cta0 = a.has_cyc && a.mode == MODE_ORTH1;
-    const int bid0 = has_ctl_cta0 ? (int)blockIdx.x - 1 : (int)blockIdx.x;
-    const int nblk = has_ctl_cta0 ? gridDim.x - 1 : gridDim.x;
-    const int64_t ngroups = (a.n + VEC - 1) / VEC;
-    const int64_t g0 = (int64_t)bid0 * THREADS + threadIdx.x;
-    double2 w0[VEC / 2];
-    if (bid0 >= 0 && g0 < ngroups && g0 * VEC + VEC <= a.n) {
+    const bool has_ctl_cta = a.has_cyc && a.mode == MODE_ORTH1;
+    const int bid = has_ctl_cta ? (int)blockIdx.x - 1 : (int)blockIdx.x;
+    const int nblk = has_ctl_cta ? gridDim.x - 1 : gridDim.x;
+    const int64_t nunits = (a.n + RT - 1) / RT;
+    const int64_t g0 = (int64_t)bid * THREADS + threadIdx.x;
+    double2 w0[RT / 2];
+    if (bid >= 0 && g0 < nunits && g0 * RT + RT <= a.n) {
 #pragma unroll
-        for (int r = 0; r < VEC; r += 2) w0[r / 2] = *reinterpret_cast<const double2 *>(a.w + g0 * VEC + r);
+        for (int r = 0; r < RT; r += 2) w0[r / 2] = *reinterpret_cast<const double2 *>(a.w + g0 * RT + r);
     }
     const int stop_after = (a.mode != MODE_HOOK) ? __ldcg(&a.ctl->stop_after) : 0;
     const double hn_dev = a.d_hn ? __ldcg(a.d_hn) : 0.0, amax_dev = a.d_amax ? __ldcg(a.d_amax) : 0.0;
     if (a.mode != MODE_HOOK && a.step > stop_after) return;
-    const bool has_ctl_cta = a.has_cyc && a.mode == MODE_ORTH1;
     if (has_ctl_cta && blockIdx.x == 0) { // the control CTA: first to be scheduled, its serial chain overlaps the streaming
         givens_step(a);
         return;
     }
-    const int bid = has_ctl_cta ? blockIdx.x - 1 : blockIdx.x;
     const double hn = a.d_hn ? hn_dev : a.hn_host;
     const double amax_w = a.d_amax ? amax_dev : a.amax_host;
     if (!(hn > 0.0)) return; // Fig. 1 l.12: h_{j+1,j} = 0 -> no new vector
@@ -133,68 +138,100 @@ template <int FMT, int THREADS> __global__ void __launch_bounds__(THREADS) store
     }
     if (bid == 0 && threadIdx.x == 0) *a.scale_out = sigma;
 
-    for (int64_t g = g0; g < ngroups; g += (int64_t)nblk * THREADS) {
-        const int64_t row = g * VEC;
-        if (row + VEC <= a.n) {
-            double v[VEC];
+    for (int64_t g = g0; g < nunits; g += (int64_t)nblk * THREADS) {
+        const int64_t row = g * RT;
+        if (row + RT <= a.n) {
+            double v[RT];
 #pragma unroll
-            for (int r = 0; r < VEC; r += 2) {
+            for (int r = 0; r < RT; r += 2) {
                 const double2 t = (g == g0) ? w0[r / 2] : *reinterpret_cast<const double2 *>(a.w + row + r);
                 v[r] = t.x / hn; // IEEE division per element (reading Q8)
                 v[r + 1] = t.y / hn;
             }
             if (a.v_out) {
+                if constexpr (BJ) {
 #pragma unroll
-                for (int r = 0; r < VEC; r += 2)
-                    *reinterpret_cast<double2 *>(a.v_out + row + r) = make_double2(v[r], v[r + 1]);
+                    for (int q = 0; q < RT / 4; ++q) { // z = A_bb^-1 v_b for the blocks this thread holds
+                        const double2 *iv = reinterpret_cast<const double2 *>(a.bj_inv + (row / 4 + q) * 16);
+                        double2 m[8];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) m[i] = __ldg(iv + i); // written once per solve, before the cycle loop
+                        double z[4];
+#pragma unroll
+                        for (int r = 0; r < 4; ++r)
+                            z[r] = fma(m[2 * r + 1].y, v[4 * q + 3], fma(m[2 * r + 1].x, v[4 * q + 2], fma(m[2 * r].y, v[4 * q + 1], m[2 * r].x * v[4 * q])));
+                        *reinterpret_cast<double2 *>(a.v_out + row + 4 * q) = make_double2(z[0], z[1]);
+                        *reinterpret_cast<double2 *>(a.v_out + row + 4 * q + 2) = make_double2(z[2], z[3]);
+                    }
+                } else {
+#pragma unroll
+                    for (int r = 0; r < RT; r += 2)
+                        *reinterpret_cast<double2 *>(a.v_out + row + r) = make_double2(v[r], v[r + 1]);
+                }
             }
-            uint4 out;
-            if constexpr (FMT == CBGMRES_FP64) {
-                out.x = (unsigned)__double2loint(v[0]);
-                out.y = (unsigned)__double2hiint(v[0]);
-                out.z = (unsigned)__double2loint(v[1]);
-                out.w = (unsigned)__double2hiint(v[1]);
-            } else if constexpr (VEC == 4) {
-                out.x = enc_bits<FMT>(v[0], s);
-                out.y = enc_bits<FMT>(v[1], s);
-                out.z = enc_bits<FMT>(v[2], s);
-                out.w = enc_bits<FMT>(v[3], s);
-            } else {
-                out.x = enc_bits<FMT>(v[0], s) | (enc_bits<FMT>(v[1], s) << 16);
-                out.y = enc_bits<FMT>(v[2], s) | (enc_bits<FMT>(v[3], s) << 16);
-                out.z = enc_bits<FMT>(v[4], s) | (enc_bits<FMT>(v[5], s) << 16);
-                out.w = enc_bits<FMT>(v[6], s) | (enc_bits<FMT>(v[7], s) << 16);
+#pragma unroll
+            for (int q = 0; q < GROUPS; ++q) {
+                const double *vq = v + q * VEC;
+                uint4 out;
+                if constexpr (FMT == CBGMRES_FP64) {
+                    out.x = (unsigned)__double2loint(vq[0]);
+                    out.y = (unsigned)__double2hiint(vq[0]);
+                    out.z = (unsigned)__double2loint(vq[1]);
+                    out.w = (unsigned)__double2hiint(vq[1]);
+                } else if constexpr (VEC == 4) {
+                    out.x = enc_bits<FMT>(vq[0], s);
+                    out.y = enc_bits<FMT>(vq[1], s);
+                    out.z = enc_bits<FMT>(vq[2], s);
+                    out.w = enc_bits<FMT>(vq[3], s);
+                } else {
+                    out.x = enc_bits<FMT>(vq[0], s) | (enc_bits<FMT>(vq[1], s) << 16);
+                    out.y = enc_bits<FMT>(vq[2], s) | (enc_bits<FMT>(vq[3], s) << 16);
+                    out.z = enc_bits<FMT>(vq[4], s) | (enc_bits<FMT>(vq[5], s) << 16);
+                    out.w = enc_bits<FMT>(vq[6], s) | (enc_bits<FMT>(vq[7], s) << 16);
+                }
+                *reinterpret_cast<uint4 *>(reinterpret_cast<char *>(a.payload) + (g * GROUPS + q) * 16) = out;
             }
-            *reinterpret_cast<uint4 *>(reinterpret_cast<char *>(a.payload) + g * 16) = out;
-        } else {
-            for (int r = 0; r < VEC && row + r < a.n; ++r) {
-                const double v = a.w[row + r] / hn;
-                if (a.v_out) a.v_out[row + r] = v;
-                if constexpr (FMT == CBGMRES_FP64) reinterpret_cast<double *>(a.payload)[row + r] = v;
-                else if constexpr (F::BYTES == 4) reinterpret_cast<unsigned *>(a.payload)[row + r] = enc_bits<FMT>(v, s);
-                else reinterpret_cast<unsigned short *>(a.payload)[row + r] = (unsigned short)enc_bits<FMT>(v, s);
+        } else { // the last, incomplete unit: row by row
+            double v[RT];
+            for (int r = 0; r < RT && row + r < a.n; ++r) {
+                v[r] = a.w[row + r] / hn;
+                if (a.v_out && !BJ) a.v_out[row + r] = v[r];
+                if constexpr (FMT == CBGMRES_FP64) reinterpret_cast<double *>(a.payload)[row + r] = v[r];
+                else if constexpr (F::BYTES == 4) reinterpret_cast<unsigned *>(a.payload)[row + r] = enc_bits<FMT>(v[r], s);
+                else reinterpret_cast<unsigned short *>(a.payload)[row + r] = (unsigned short)enc_bits<FMT>(v[r], s);
+            }
+            if (BJ && a.v_out) { // the last block is completed by the identity: only its real rows and columns count
+                for (int r = 0; r < RT && row + r < a.n; ++r) {
+                    const int q = r / 4;
+                    const double *iv = a.bj_inv + (row / 4 + q) * 16 + (r & 3) * 4;
+                    double z = 0.0;
+                    for (int c = 0; c < 4 && row + 4 * q + c < a.n; ++c) z = fma(iv[c], v[4 * q + c], z);
+                    a.v_out[row + r] = z;
+                }
             }
         }
     }
 }
 
-template <int FMT> static int launch_store_t(cudaStream_t s, const StoreArgs &a)
+template <int FMT> static int launch_store_t(cudaStream_t s, const Scratch &sc, const StoreArgs &a)
 {
     constexpr int THREADS = 256;
     using F = Fmt<FMT>;
-    const int64_t ngroups = (a.n + F::VEC - 1) / F::VEC;
-    int64_t grid = (ngroups + THREADS - 1) / THREADS;
+    const int RT = (a.bj_inv && F::VEC < 4) ? 4 : F::VEC;
+    const int64_t nunits = (a.n + RT - 1) / RT;
+    int64_t grid = (nunits + THREADS - 1) / THREADS;
     const int64_t cap = (int64_t)kNumSMs * 8;
     if (grid > cap) grid = cap;
     if (grid < 1) grid = 1;
     if (a.has_cyc && a.mode == MODE_ORTH1) grid += 1; // + the control CTA (Givens update)
-    launch_chain(store_kernel<FMT, THREADS>, dim3((unsigned)grid), dim3(THREADS), 0, s, a);
+    if (a.bj_inv) launch_chain(sc, "store_kernel", store_kernel<FMT, THREADS, true>, dim3((unsigned)grid), dim3(THREADS), 0, s, a);
+    else launch_chain(sc, "store_kernel", store_kernel<FMT, THREADS, false>, dim3((unsigned)grid), dim3(THREADS), 0, s, a);
     return 1;
 }
 
 int launch_store(cudaStream_t s, const Scratch &sc, int format, int64_t n, const double *w, const double *d_hn,
                  const double *d_amax, double hn_host, double amax_host, void *payload_col, double *scale_out,
-                 double *v_out, int mode, int step, const CycleState *cyc, int *h_flag)
+                 double *v_out, int mode, int step, const CycleState *cyc, int *h_flag, const double *bj_inv)
 {
     StoreArgs a{};
     a.w = w;
@@ -212,12 +249,13 @@ int launch_store(cudaStream_t s, const Scratch &sc, int format, int64_t n, const
     a.mode = mode;
     a.step = step;
     a.h_flag = h_flag;
+    a.bj_inv = bj_inv;
     switch (format) {
-    case CBGMRES_FP64: return launch_store_t<CBGMRES_FP64>(s, a);
-    case CBGMRES_FP32: return launch_store_t<CBGMRES_FP32>(s, a);
-    case CBGMRES_FP16: return launch_store_t<CBGMRES_FP16>(s, a);
-    case CBGMRES_INT32: return launch_store_t<CBGMRES_INT32>(s, a);
-    case CBGMRES_INT16: return launch_store_t<CBGMRES_INT16>(s, a);
+    case CBGMRES_FP64: return launch_store_t<CBGMRES_FP64>(s, sc, a);
+    case CBGMRES_FP32: return launch_store_t<CBGMRES_FP32>(s, sc, a);
+    case CBGMRES_FP16: return launch_store_t<CBGMRES_FP16>(s, sc, a);
+    case CBGMRES_INT32: return launch_store_t<CBGMRES_INT32>(s, sc, a);
+    case CBGMRES_INT16: return launch_store_t<CBGMRES_INT16>(s, sc, a);
     default: return 0;
     }
 }

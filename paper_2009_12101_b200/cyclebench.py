@@ -34,9 +34,42 @@ def cycle_bytes(n: int, nnz: int, m: int, fmt: str, reorth_share: float) -> floa
     return steps + model.update_bytes(n, m, fmt) + model.spmv_bytes(n, nnz) + 8 * n + model.store_bytes(n, fmt)
 
 
-def main(argv=None) -> int:
+def run(s, p, ms, cycles, fmts, reorth="cond", out=None):
+    """The sweep on handle `s` (matrix of problem `p` already registered).  Returns the rows."""
     import torch
 
+    n, nnz = p.A.n, p.A.nnz
+    b = torch.as_tensor(p.b, device=s.device)
+    x0 = torch.as_tensor(p.x0, device=s.device)
+    rows = []
+    for m in ms:
+        base_ms = base_bytes = None
+        for fmt in fmts:
+            iters = cycles * m
+            s.solve(b, x0, m, 0.0, m, fmt, reorth=reorth)  # warm-up: one cycle
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            _, r = s.solve(b, x0, m, 0.0, iters, fmt, reorth=reorth)
+            e1.record()
+            e1.synchronize()
+            cyc = max(1, r.iters // m)
+            per_cycle = e0.elapsed_time(e1) / cyc
+            share = r.reorth_count / max(1, r.iters)
+            by = cycle_bytes(n, nnz, m, fmt, share)
+            if fmt == "fp64":
+                base_ms, base_bytes = per_cycle, by
+            row = {"m": m, "format": fmt, "iters": r.iters, "reorth_count": r.reorth_count, "ms_per_cycle": per_cycle,
+                   "us_per_step": per_cycle * 1e3 / m, "speedup_vs_fp64": base_ms / per_cycle,
+                   "bytes_ratio_vs_fp64": base_bytes / by, "GBps": by / per_cycle / 1e6}
+            rows.append(row)
+            if out:
+                out(f"{m:4d} {fmt:6s} {r.iters:6d} {r.reorth_count:6d} {per_cycle:9.3f} {row['us_per_step']:8.1f} "
+                    f"{row['speedup_vs_fp64']:8.2f} {row['bytes_ratio_vs_fp64']:11.2f} {row['GBps']:7.0f}")
+    return rows
+
+
+def main(argv=None) -> int:
     from workloads import make_config
 
     ap = argparse.ArgumentParser()
@@ -56,34 +89,9 @@ def main(argv=None) -> int:
     n, nnz = p.A.n, p.A.nnz
     s = Solver(0)
     s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
-    b = torch.as_tensor(p.b, device=s.device)
-    x0 = torch.as_tensor(p.x0, device=s.device)
-    rows = []
     print(f"# {args.workload}: n={n} nnz={nnz} cycles={args.cycles} reorth={args.reorth} (tolerance 0: fixed iteration count)")
     print(f"{'m':>4s} {'fmt':6s} {'iters':>6s} {'reorth':>6s} {'ms/cycle':>9s} {'us/step':>8s} {'speedup':>8s} {'bytes ratio':>11s} {'GB/s':>7s}")
-    for m in ms:
-        base_ms = base_bytes = None
-        for fmt in fmts:
-            iters = args.cycles * m
-            s.solve(b, x0, m, 0.0, m, fmt, reorth=args.reorth)  # warm-up: one cycle
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda.synchronize()
-            e0.record()
-            _, r = s.solve(b, x0, m, 0.0, iters, fmt, reorth=args.reorth)
-            e1.record()
-            e1.synchronize()
-            cyc = max(1, r.iters // m)
-            per_cycle = e0.elapsed_time(e1) / cyc
-            share = r.reorth_count / max(1, r.iters)
-            by = cycle_bytes(n, nnz, m, fmt, share)
-            if fmt == "fp64":
-                base_ms, base_bytes = per_cycle, by
-            row = {"m": m, "format": fmt, "iters": r.iters, "reorth_count": r.reorth_count, "ms_per_cycle": per_cycle,
-                   "us_per_step": per_cycle * 1e3 / m, "speedup_vs_fp64": base_ms / per_cycle,
-                   "bytes_ratio_vs_fp64": base_bytes / by, "GBps": by / per_cycle / 1e6}
-            rows.append(row)
-            print(f"{m:4d} {fmt:6s} {r.iters:6d} {r.reorth_count:6d} {per_cycle:9.3f} {row['us_per_step']:8.1f} "
-                  f"{row['speedup_vs_fp64']:8.2f} {row['bytes_ratio_vs_fp64']:11.2f} {row['GBps']:7.0f}")
+    rows = run(s, p, ms, args.cycles, fmts, args.reorth, out=print)
     if args.json:
         with open(args.json, "w") as f:
             json.dump({"workload": args.workload, "n": n, "nnz": nnz, "cycles": args.cycles, "reorth": args.reorth,

@@ -38,29 +38,14 @@ def _time(fn, reps, flush_buf, torch):
     return statistics.median(ts), min(ts)
 
 
-def main(argv=None) -> int:
+def run(s, n, ks, fmts, reps=20, flush=True, log=None):
+    """Times S2 (multi-dot), S3 (update + norms), the fused S3 + S2' and S4 (store) separately on handle `s`.
+    Returns a list of rows {"kernel", "format", "k", "median_us", "best_us", "bytes", "GBps"}."""
     import torch
 
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--n", type=int, default=4_194_304)
-    ap.add_argument("--k", default="1,2,4,8,16,32,64,100")
-    ap.add_argument("--formats", default=",".join(FORMATS))
-    ap.add_argument("--reps", type=int, default=20)
-    ap.add_argument("--flush", action="store_true")
-    ap.add_argument("--spmv", default="")
-    ap.add_argument("--json", default="")
-    ap.add_argument("--interleave", type=int, default=0, help="orth_interleave option: 0 auto, 1 blocked, 2 interleaved")
-    ap.add_argument("--spmv-kernel", default="0", help="comma list of spmv_kernel options to time (0 = auto)")
-    ap.add_argument("--seg-kb", type=int, default=0, help="orth_seg_kb option: 0 auto, 1, 2, 4")
-    args = ap.parse_args(argv)
-    ks = [int(x) for x in args.k.split(",") if x]
-    fmts = [f for f in args.formats.split(",") if f]
-    n, kmax = args.n, max(ks)
-    s = Solver(0)
-    s.set_option("orth_seg_kb", args.seg_kb)
-    s.set_option("orth_interleave", args.interleave)
     dev = s.device
-    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev) if args.flush else None
+    kmax = max(ks)
+    flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device=dev) if flush else None
     rows = []
     g = torch.Generator(device=dev)
     g.manual_seed(2)
@@ -77,19 +62,51 @@ def main(argv=None) -> int:
         for k in ks:
             h = s.k_multidot(fmt, V, sig, w0, n=n, k=k).clone()
             w = w0.clone()
-            med, best = _time(lambda: s.k_multidot(fmt, V, sig, w0, n=n, k=k), args.reps, flush, torch)
+            med, best = _time(lambda: s.k_multidot(fmt, V, sig, w0, n=n, k=k), reps, flush_buf, torch)
             rows.append(("multidot", fmt, k, med, best, model.multidot_bytes(n, k, fmt)))
             hz = torch.zeros_like(h)  # w -= V*0 keeps w bounded over the repetitions; same traffic and flops
-            med, best = _time(lambda: s.k_update(fmt, V[:k], sig, hz, w, n=n), args.reps, flush, torch)
+            med, best = _time(lambda: s.k_update(fmt, V[:k], sig, hz, w, n=n), reps, flush_buf, torch)
             rows.append(("update", fmt, k, med, best, model.update_bytes(n, k, fmt)))
             if k <= 128:
-                med, best = _time(lambda: s.k_update_multidot(fmt, V[:k], sig, hz, w, n=n), args.reps, flush, torch)
+                med, best = _time(lambda: s.k_update_multidot(fmt, V[:k], sig, hz, w, n=n), reps, flush_buf, torch)
                 rows.append(("update_multidot", fmt, k, med, best, model.update_bytes(n, k, fmt)))
         col = torch.empty(ld, dtype=payload_dtype(fmt), device=dev)
         vout = torch.empty(n, dtype=torch.float64, device=dev)
-        med, best = _time(lambda: s.k_store(fmt, w0, 2.0, 6.0, col, vout), args.reps, flush, torch)
+        med, best = _time(lambda: s.k_store(fmt, w0, 2.0, 6.0, col, vout), reps, flush_buf, torch)
         rows.append(("store", fmt, 1, med, best, model.store_bytes(n, fmt)))
         del V
+        if log:
+            log(f"microbench {fmt} done")
+    return [{"kernel": name, "format": fmt, "k": k, "median_us": med * 1e6, "best_us": best * 1e6, "bytes": by,
+             "GBps": by / med / 1e9} for name, fmt, k, med, best, by in rows]
+
+
+def main(argv=None) -> int:
+    import torch
+
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--n", type=int, default=4_194_304)
+    ap.add_argument("--k", default="1,2,4,8,16,32,50,64,100")
+    ap.add_argument("--formats", default=",".join(FORMATS))
+    ap.add_argument("--reps", type=int, default=20)
+    ap.add_argument("--flush", action="store_true")
+    ap.add_argument("--spmv", default="")
+    ap.add_argument("--json", default="")
+    ap.add_argument("--interleave", type=int, default=0, help="orth_interleave option: 0 auto, 1 blocked, 2 interleaved")
+    ap.add_argument("--spmv-kernel", default="0", help="comma list of spmv_kernel options to time (0 = auto)")
+    ap.add_argument("--seg-kb", type=int, default=0, help="orth_seg_kb option: 0 auto, 1, 2, 4")
+    args = ap.parse_args(argv)
+    ks = [int(x) for x in args.k.split(",") if x]
+    fmts = [f for f in args.formats.split(",") if f]
+    n = args.n
+    s = Solver(0)
+    s.set_option("orth_seg_kb", args.seg_kb)
+    s.set_option("orth_interleave", args.interleave)
+    dev = s.device
+    out = run(s, n, ks, fmts, args.reps, args.flush) if ks and fmts else []
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev) if args.flush else None
+    g = torch.Generator(device=dev)
+    g.manual_seed(3)
     for name in [x for x in args.spmv.split(",") if x]:
         from workloads import make_config
 
@@ -100,14 +117,14 @@ def main(argv=None) -> int:
             s.set_option("spmv_kernel", kern)
             s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
             med, best = _time(lambda: s.k_spmv(x, y, want_norm=False), args.reps, flush, torch)
-            rows.append((f"spmv[{name},opt={kern}]", "fp64", 0, med, best, model.spmv_bytes(p.A.n, p.A.nnz)))
+            by = model.spmv_bytes(p.A.n, p.A.nnz)
+            out.append({"kernel": f"spmv[{name},opt={kern}]", "format": "fp64", "k": 0, "median_us": med * 1e6,
+                        "best_us": best * 1e6, "bytes": by, "GBps": by / med / 1e9})
     print(f"# n={n} reps={args.reps} flush={args.flush}  GB/s = algorithmic bytes / median time")
     print(f"{'kernel':28s} {'fmt':6s} {'k':>4s} {'median_us':>10s} {'best_us':>10s} {'MB':>9s} {'GB/s':>8s}")
-    out = []
-    for name, fmt, k, med, best, by in rows:
-        print(f"{name:28s} {fmt:6s} {k:4d} {med * 1e6:10.1f} {best * 1e6:10.1f} {by / 1e6:9.1f} {by / med / 1e9:8.0f}")
-        out.append({"kernel": name, "format": fmt, "k": k, "median_us": med * 1e6, "best_us": best * 1e6, "bytes": by,
-                    "GBps": by / med / 1e9})
+    for r in out:
+        print(f"{r['kernel']:28s} {r['format']:6s} {r['k']:4d} {r['median_us']:10.1f} {r['best_us']:10.1f} "
+              f"{r['bytes'] / 1e6:9.1f} {r['GBps']:8.0f}")
     if args.json:
         with open(args.json, "w") as f:
             json.dump({"n": n, "flush": args.flush, "rows": out}, f, indent=1)

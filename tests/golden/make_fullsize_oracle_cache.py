@@ -6,7 +6,7 @@ for iteration-count parity (cache its result keyed by config + format)").
 This script calls ONLY oracle/ (the plain CPU CB-GMRES written from PAPER.md, Fig. 1) and the seeded
 input generators in workloads/; nothing from the CUDA path.  Every stored value is the oracle's.
 
-    python tests/golden/make_fullsize_oracle_cache.py [--cases C2,C5,C4J,C4] [--spread 7,6,5,4]
+    python tests/golden/make_fullsize_oracle_cache.py [--cases C2,C5,C4J,C4B,C4] [--spread 7,6,5,4]
                                                       [--formats fp64,...] [--out path]
 
 Per case and storage format it stores the result of the base run (oracle at BASE_THREADS threads):
@@ -50,6 +50,8 @@ CASES = {
     # instead of the config's 5,000: int16 does not converge on this matrix,
     # both sides then stop at the bound and 4,000 more oracle steps would pin nothing more.
     "C4J": ("C4", "jacobi", 1000),
+    # C4 with the block-Jacobi(4) preconditioner of the paper's section 6.5, same bound.
+    "C4B": ("C4", "block_jacobi4", 1000),
     # C4 as BASELINE.json states it (no preconditioner): does not converge (reading Q12); both sides stop
     # at a short bound with comparable residuals.
     "C4": ("C4", "none", 150),
@@ -74,7 +76,7 @@ def save(path, data):
 
 def main(argv=None) -> int:
     ap = argparse.ArgumentParser()
-    ap.add_argument("--cases", default="C2,C5,C4J,C4")
+    ap.add_argument("--cases", default="C2,C5,C4J,C4B,C4")
     ap.add_argument("--formats", default=",".join(oracle.FORMATS))
     ap.add_argument("--spread", default="7,6,5,4", help="thread counts of the extra runs of the quantised formats")
     ap.add_argument("--out", default=OUT)

@@ -6,7 +6,11 @@ residual histories over a bounded prefix of the solve)."""
 import numpy as np
 import pytest
 
+import json
+import os
+
 import oracle
+from parity import check_iters
 from workloads import make_config
 
 pytestmark = pytest.mark.gpu
@@ -44,7 +48,7 @@ def c3_vectors():
     return V, w, h
 
 
-@pytest.mark.parametrize("fmt", ["fp32", "int16"])
+@pytest.mark.parametrize("fmt", oracle.FORMATS)
 def test_c3_size_passes_sampled(solver, c3_vectors, fmt):
     import torch
     from paper_2009_12101_b200 import payload_dtype
@@ -159,3 +163,69 @@ def test_full_size_c2_residual_history_prefix(c2_full, fmt):
     hg, ho = np.asarray(r.rec_history[:steps]), np.asarray(ref.rec_history[:steps])
     assert np.all(np.abs(hg - ho) <= HIST_TOL[fmt] * ho)
     assert r.reorth_count == ref.reorth_count
+
+
+# ---- full-size solves to convergence against the oracle's cached results -----------------------------------------
+# tests/golden/fullsize_oracle.json is written by tests/golden/make_fullsize_oracle_cache.py, which calls only
+# oracle/ (hours of CPU work: SURVEY.md 8(d) "cache its result keyed by config + format").  north_star: iteration
+# counts to convergence within +-2 %, true residuals both below the tolerance and within 10x of each other.
+_CACHE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "fullsize_oracle.json")
+_PRECOND = {"C2": "none", "C5": "none", "C4J": "jacobi", "C4B": "block_jacobi4", "C4": "none"}
+
+
+def _cached(case, fmt):
+    if not os.path.exists(_CACHE):
+        pytest.fail("tests/golden/fullsize_oracle.json is missing: run tests/golden/make_fullsize_oracle_cache.py")
+    with open(_CACHE) as f:
+        data = json.load(f)
+    entry = data["cases"].get(case)
+    if entry is None or "iters" not in entry["formats"].get(fmt, {}):
+        pytest.skip(f"{case} {fmt}: no cached oracle result")
+    return entry, entry["formats"][fmt]
+
+
+@pytest.fixture(scope="module")
+def full_solvers():
+    """One handle + matrix per full-size config, made on first use and kept for the module."""
+    from paper_2009_12101_b200 import Solver
+
+    made = {}
+
+    def get(cfg):
+        if cfg not in made:
+            p = make_config(cfg)
+            s = Solver(0)
+            s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+            made[cfg] = (p, s)
+        return made[cfg]
+
+    yield get
+    for _, s in made.values():
+        s.destroy()
+
+
+@pytest.mark.parametrize("fmt", oracle.FORMATS)
+@pytest.mark.parametrize("case", ["C2", "C5", "C4J", "C4B", "C4"])
+def test_full_size_solve_matches_cached_oracle(full_solvers, case, fmt):
+    entry, o = _cached(case, fmt)
+    p, s = full_solvers(entry["config"])
+    assert (p.A.n, p.A.nnz, p.restart, p.rel_tol) == (entry["n"], entry["nnz"], entry["restart"], entry["rel_tol"])
+    x, r = s.solve(p.b, p.x0, p.restart, p.rel_tol, entry["max_iters"], fmt, precond=_PRECOND[case], history=True)
+    xh = x.cpu().numpy()
+    true = np.linalg.norm(p.b - oracle.spmv(p.A, xh)) / np.linalg.norm(p.b)  # recomputed with the oracle's SpMV
+    assert bool(r.converged) == o["converged"], (case, fmt, r.iters, o["iters"])
+    draws = [d["iters"] for d in o.get("spread", {}).values()]
+    rule = check_iters(r.iters, o["iters"], fmt, case, draws=draws if draws else None)
+    assert r.rel_res_true == pytest.approx(true, rel=1e-6)
+    if o["converged"]:
+        assert true <= p.rel_tol * (1 + 1e-9) and o["rel_res_true_recomputed"] <= p.rel_tol * (1 + 1e-9)
+    assert true <= 10 * o["rel_res_true_recomputed"] and o["rel_res_true_recomputed"] <= 10 * true
+    if rule == "strict":
+        assert abs(r.restarts - o["restarts"]) <= 1
+        assert abs(r.reorth_count - o["reorth_count"]) <= max(2, 0.02 * o["reorth_count"])
+    # the first 40 steps are before any decorrelation: the recurrence residuals agree to the format's roundoff
+    k = min(40, r.iters, o["iters"])
+    hg, ho = np.asarray(r.rec_history[:k]), np.asarray(o["rec_history"][:k])
+    assert np.all(np.abs(hg - ho) <= HIST_TOL[fmt] * ho * (100 if case.startswith("C4") else 1))
+    print(f"[full-size] {case} {fmt}: gpu iters {r.iters} restarts {r.restarts} | oracle {o['iters']} {o['restarts']} "
+          f"draws {sorted(draws)} | rule {rule} | true residual gpu {true:.3e} oracle {o['rel_res_true_recomputed']:.3e}")

@@ -119,6 +119,55 @@ def test_store_normalises_and_compresses(solver, fmt, n):
     assert s.item() == exp_s
 
 
+# ------------------------------------------------------------------------------------------ block-Jacobi(4)
+@pytest.mark.parametrize("cfg,kw", [("C5", {"grid": 12}), ("C4", {"n": 5003}), ("C2", {"grid": 11}), ("C1", {"grid": 5})])
+def test_bj4_setup_matches_oracle_blocks(cfg, kw):
+    """The inverted 4 x 4 diagonal blocks of stencil and power-law matrices, ragged last blocks
+    included (n = 5003, 1331, 25), against the oracle's Gauss-Jordan inverses."""
+    from paper_2009_12101_b200 import Solver
+
+    p = make_config(cfg, **kw)
+    s = Solver(0)
+    try:
+        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+        got = s.k_bj4_setup().cpu().numpy()
+    finally:
+        s.destroy()
+    exp = oracle.block_jacobi4(p.A)
+    assert got.shape == exp.shape
+    scale = np.abs(exp).max(axis=(1, 2), keepdims=True)
+    assert np.all(np.abs(got - exp) <= 1e-12 * scale)
+    r = p.A.n % 4
+    if r:  # identity completion of the last block, bit for bit
+        assert np.array_equal(got[-1, r:, :], exp[-1, r:, :]) and np.array_equal(got[-1, :, r:], exp[-1, :, r:])
+
+
+@pytest.mark.parametrize("fmt", FORMATS)
+@pytest.mark.parametrize("n", [1, 3, 4, 7, 4099, 70002])
+def test_store_bj4_compresses_v_and_hands_minv_v_to_the_spmv(solver, fmt, n):
+    """S4 under block-Jacobi: the payload is still enc(v), bit-exact; the fp64 output is z = M^-1 v (Fig. 1 l.3)."""
+    rng = np.random.default_rng(300 + n)
+    w = rng.standard_normal(n) * 3.5
+    hn, amax = float(np.linalg.norm(w)), float(np.abs(w).max())
+    v = w / hn
+    nb = (n + 3) // 4
+    inv = rng.standard_normal((nb, 4, 4)) * 10.0 ** rng.uniform(-2, 2, (nb, 1, 1))
+    if n % 4:
+        r = n % 4
+        inv[-1, r:, :] = 0.0
+        inv[-1, :, r:] = 0.0
+        inv[-1, np.arange(r, 4), np.arange(r, 4)] = 1.0
+    exp_p, exp_s = oracle.enc(fmt, v)
+    z_ref = oracle.apply_minv("block_jacobi4", inv, v)
+    vpad = np.zeros(4 * nb)
+    vpad[:n] = v
+    zabs = np.einsum("brc,bc->br", np.abs(inv), np.abs(vpad.reshape(nb, 4))).ravel()[:n]
+    pl, sc, z = solver.k_store_bj4(fmt, _dev(w), hn, amax, _dev(inv))
+    assert np.array_equal(pl.cpu().numpy().view(np.uint8), exp_p.view(np.uint8))
+    assert sc.item() == exp_s
+    assert np.all(np.abs(z.cpu().numpy() - z_ref) <= TOL * np.maximum(zabs, 1e-300))
+
+
 # ------------------------------------------------------------------------------------------ multi-dot / update
 @pytest.mark.parametrize("fmt", FORMATS)
 @pytest.mark.parametrize("n,k", [(1, 1), (63, 3), (4096, 8), (50021, 1), (50021, 9), (50021, 33), (200003, 100)])

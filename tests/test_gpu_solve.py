@@ -6,6 +6,7 @@ import numpy as np
 import pytest
 
 import oracle
+from parity import check_iters
 from workloads import make_config, random_dense_system
 
 pytestmark = pytest.mark.gpu
@@ -29,46 +30,23 @@ def _true_rel_res(p, x):
     return oracle.nrm2(p.b - oracle.spmv(p.A, x)) / oracle.nrm2(p.b)
 
 
-def _assert_iters_parity(gpu_iters, ref, p, fmt, restart, rel_tol, max_iters, reorth, precond="none"):
-    """+-2 % (at least +-2 steps) of the oracle's iteration count.  With a quantised basis the store
-    is a discontinuous map: a last-bit difference in one inner product flips rounding decisions and
-    the two residual histories decorrelate at the level of the storage format's unit roundoff after
-    some tens of steps (measured: DESIGN.md reading Q11).  Where the FIRST comparison fails, the
-    band is therefore widened to the spread of the oracle's OWN counts when only the order of its
-    block sums changes (thread counts 1, 2, 3, 5) -- nothing else about the oracle changes.  Five
-    draws under-estimate the range of a wide distribution (a sixth independent draw falls outside the
-    range of five with probability 2/6), so the band is that range extended by two sample standard
-    deviations of the oracle's own counts; when they coincide this is the plain +-2 %."""
-    tol = lambda c: max(2, 0.02 * c)
-    if abs(gpu_iters - ref.iters) <= tol(ref.iters):
-        return
-    assert fmt != "fp64", ("fp64 storage has no quantisation: no band", gpu_iters, ref.iters)
-    counts = [ref.iters]
-    base = oracle.num_threads()
-    try:
-        for t in (1, 2, 3, 5):
-            oracle.set_num_threads(t)
-            counts.append(oracle.gmres(p.A, p.b, p.x0, restart, rel_tol, max_iters, fmt, reorth=reorth,
-                                       precond=precond).iters)
-    finally:
-        oracle.set_num_threads(base)
-    lo, hi, sd = min(counts), max(counts), float(np.std(counts, ddof=1))
-    assert lo - max(tol(lo), 2 * sd) <= gpu_iters <= hi + max(tol(hi), 2 * sd), (fmt, gpu_iters, counts)
-
-
-def _check_parity(p, fmt, restart=None, rel_tol=None, max_iters=None, reorth="cond", precond="none"):
+def _check_parity(p, fmt, restart=None, rel_tol=None, max_iters=None, reorth="cond", precond="none", label=None):
+    """GPU solve against the oracle's: counts through the shared checker (tests/parity.py: strict +-2 %, the
+    oracle's own spread for quantised formats, the listed chaotic cases), residuals, restarts, ||b||."""
     restart, rel_tol, max_iters = restart or p.restart, rel_tol or p.rel_tol, max_iters or p.max_iters
-    ref = oracle.gmres(p.A, p.b, p.x0, restart, rel_tol, max_iters, fmt, reorth=reorth, precond=precond)
+    label = label or p.name
+    run = lambda: oracle.gmres(p.A, p.b, p.x0, restart, rel_tol, max_iters, fmt, reorth=reorth, precond=precond)
+    ref = run()
     x, r = _solve_gpu(p, fmt, restart, rel_tol, max_iters, reorth, precond=precond)
     true_gpu = _true_rel_res(p, x)
     true_ref = _true_rel_res(p, ref.x)
     assert r.converged == ref.converged
-    _assert_iters_parity(r.iters, ref, p, fmt, restart, rel_tol, max_iters, reorth, precond)
+    rule = check_iters(r.iters, ref.iters, fmt, label, run=run)
     if ref.converged:
         assert true_gpu <= rel_tol * (1 + 1e-9) and true_ref <= rel_tol * (1 + 1e-9)
     assert true_gpu <= 10 * true_ref and true_ref <= 10 * true_gpu
     assert r.rel_res_true == pytest.approx(true_gpu, rel=1e-6)
-    if abs(r.iters - ref.iters) <= max(2, 0.02 * ref.iters):  # cycles are comparable only where the counts are
+    if rule == "strict":  # cycles are comparable only where the counts are
         assert abs(r.restarts - ref.restarts) <= 1
     assert r.b_norm == pytest.approx(ref.b_norm, rel=1e-13)
     return r, ref
@@ -83,14 +61,14 @@ def test_c1_full_size(fmt):
 
 @pytest.mark.parametrize("fmt", oracle.FORMATS)
 def test_c2_reduced(fmt):
-    _check_parity(make_config("C2", grid=32), fmt)
+    _check_parity(make_config("C2", grid=32), fmt, label="C2-32")
 
 
 @pytest.mark.parametrize("fmt", oracle.FORMATS)
 def test_c4_reduced(fmt):
     # without a preconditioner C4 does not converge within its iteration bound (reading Q12); both
     # sides must then stop at the bound with comparable true residuals
-    r, ref = _check_parity(make_config("C4", n=40000), fmt, max_iters=300)
+    r, ref = _check_parity(make_config("C4", n=40000), fmt, max_iters=300, label="C4-40k")
     assert r.iters == ref.iters == 300
 
 
@@ -98,7 +76,7 @@ def test_c4_reduced(fmt):
 def test_c4_reduced_jacobi_converges(fmt):
     """The paper's default preconditioner (scalar Jacobi) as the right preconditioner of
     Fig. 1 l.3 / l.17: C4 converges on both sides, counts and residuals as in every other parity case."""
-    r, ref = _check_parity(make_config("C4", n=40000), fmt, max_iters=2000, precond="jacobi")
+    r, ref = _check_parity(make_config("C4", n=40000), fmt, max_iters=2000, precond="jacobi", label="C4J-40k")
     assert r.converged and ref.converged
 
 
@@ -107,7 +85,7 @@ def test_c2_reduced_jacobi_constant_diagonal(fmt):
     """C2's diagonal is the constant 6: A D^-1 = A / 6, same Krylov spaces (streamed SpMV variant with
     the scaled copy of the values; x = D^-1 u at the end)."""
     p = make_config("C2", grid=32)
-    r, ref = _check_parity(p, fmt, precond="jacobi")
+    r, ref = _check_parity(p, fmt, precond="jacobi", label="C2J-32")
     _, plain = _solve_gpu(p, fmt)
     assert r.converged and abs(r.iters - plain.iters) <= max(2, 0.02 * plain.iters)
 
@@ -149,13 +127,13 @@ def test_jacobi_host_entry_and_workspace():
 
 @pytest.mark.parametrize("fmt", oracle.FORMATS)
 def test_c5_reduced(fmt):
-    _check_parity(make_config("C5", grid=24), fmt)
+    _check_parity(make_config("C5", grid=24), fmt, label="C5-24")
 
 
 @pytest.mark.parametrize("reorth", ["never", "always"])
 def test_reorth_modes(reorth):
     p = make_config("C2", grid=20)
-    r, ref = _check_parity(p, "fp32", restart=30, reorth=reorth)
+    r, ref = _check_parity(p, "fp32", restart=30, reorth=reorth, label="C2-20-" + reorth)
     assert (r.reorth_count == 0) if reorth == "never" else (r.reorth_count == r.iters)
 
 
@@ -301,3 +279,214 @@ def test_measurement_drivers_run(capsys):
     assert paperprotocol.main(["--small", "--max-iters", "3000"]) == 0
     out = capsys.readouterr().out
     assert "fp32" in out and "3/3" in out
+
+
+# ---- block-Jacobi(4) right preconditioner -----------------------------------
+
+@pytest.mark.parametrize("fmt", oracle.FORMATS)
+def test_c4_reduced_block_jacobi4(fmt):
+    """C4 (power-law rows, strongly varying diagonal) with M = the 4 x 4 diagonal blocks: converges on both
+    sides; counts, residuals and restarts as in every other parity case."""
+    r, ref = _check_parity(make_config("C4", n=40000), fmt, max_iters=2000, precond="block_jacobi4", label="C4B-40k")
+    assert r.converged and ref.converged
+
+
+@pytest.mark.parametrize("fmt", oracle.FORMATS)
+def test_c5_reduced_block_jacobi4(fmt):
+    """27-point stencil: four consecutive grid points are coupled, so the blocks are genuinely 4 x 4."""
+    r, ref = _check_parity(make_config("C5", grid=24), fmt, precond="block_jacobi4", label="C5B-24")
+    assert r.converged
+
+
+@pytest.mark.parametrize("fmt", ["fp64", "int16"])
+def test_c2_reduced_block_jacobi4_ragged_last_block(fmt):
+    """n = 27^3 = 19683 = 4 * 4920 + 3: the last block has three rows (identity completion); streamed SpMV
+    of z = M^-1 v written by the store kernel's scalar tail."""
+    _check_parity(make_config("C2", grid=27), fmt, precond="block_jacobi4", label="C2B-27")
+
+
+def test_block_jacobi4_tiny_dense_nonzero_x0_matches_direct_solve():
+    import scipy.sparse as sp
+    from workloads import CSR, Problem
+
+    n = 50  # ragged last block (2 rows)
+    rng = np.random.default_rng(64)
+    M = np.zeros((n, n))
+    for b0 in range(0, n, 4):
+        b1 = min(n, b0 + 4)
+        blk = 0.3 * rng.standard_normal((b1 - b0, b1 - b0)) + 2.0 * np.eye(b1 - b0)[::-1] + 0.5 * np.eye(b1 - b0)
+        M[b0:b1, b0:b1] = 10.0 ** rng.uniform(-1.0, 1.0) * blk
+    Ad = (np.eye(n) + 0.05 * rng.standard_normal((n, n))) @ M
+    S = sp.csr_matrix(Ad)
+    S.sort_indices()
+    A = CSR(n, S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(np.float64))
+    b, x0 = rng.standard_normal(n), rng.standard_normal(n)
+    p = Problem("tinyB", A, b, x0, n, 1e-11, 4 * n, ("fp64",), {})
+    x, r = _solve_gpu(p, "fp64", precond="block_jacobi4")
+    ref = oracle.gmres(A, b, x0, n, 1e-11, 4 * n, "fp64", precond="block_jacobi4")
+    xs = np.linalg.solve(Ad, b)
+    assert r.converged and ref.converged and r.iters == ref.iters and r.iters <= n
+    assert np.linalg.norm(x - xs) <= 1e-8 * np.linalg.norm(xs)
+    assert _true_rel_res(p, x) <= 1e-11 * (1 + 1e-6)
+    # scalar Jacobi and no preconditioner do far worse on this matrix: the blocks are what is applied
+    _, rj = _solve_gpu(p, "fp64", precond="jacobi", restart=10, max_iters=300)
+    _, rb = _solve_gpu(p, "fp64", precond="block_jacobi4", restart=10, max_iters=300)
+    assert rb.converged and ((not rj.converged) or rj.iters > 2 * rb.iters)
+
+
+def test_block_jacobi4_host_entry_and_workspace():
+    from paper_2009_12101_b200 import Solver
+
+    p = make_config("C4", n=20001)
+    s = Solver(0)
+    try:
+        x = p.x0.copy()
+        r = s.solve_host(p.A.row_ptr, p.A.col_idx, p.A.vals, p.b, x, p.restart, p.rel_tol, 2000, "fp32", precond="block_jacobi4")
+        assert r.converged and _true_rel_res(p, x) <= p.rel_tol * (1 + 1e-6)
+        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+        assert s.workspace_bytes(p.restart, "fp32", precond="block_jacobi4") >= s.workspace_bytes(p.restart, "fp32") + 128 * ((p.A.n + 3) // 4)
+    finally:
+        s.destroy()
+
+
+# ---- Fig. 1 l.12: the second pass again lost more than eta (reading Q4; oracle pin in test_oracle_gmres.py) ------
+
+@pytest.mark.parametrize("fmt,u", [("fp32", 2.0 ** -24), ("fp16", 2.0 ** -11), ("int32", 2.0 ** -31), ("int16", 2.0 ** -15)])
+def test_second_pass_breakdown_clause_matches_oracle(fmt, u):
+    """A = blockdiag(A1, I), b in the first d coordinates: the Krylov space closes at dimension d; with a
+    quantised basis h_{d+1,d} stays nonzero (about u^2 omega) and only the clause hn < eta * omega1 of l.12 ends
+    the cycle there.  tau = 0 is out of reach, so the recurrence test cannot end it."""
+    import scipy.sparse as sp
+    from workloads import CSR, Problem
+
+    n, d, m = 40, 6, 20
+    rng = np.random.default_rng(95)
+    A1 = rng.standard_normal((d, d)) + d * np.eye(d)
+    Ad = np.eye(n)
+    Ad[:d, :d] = A1
+    b = np.zeros(n)
+    b[:d] = rng.standard_normal(d)
+    xs = np.zeros(n)
+    xs[:d] = np.linalg.solve(A1, b[:d])
+    S = sp.csr_matrix(Ad)
+    S.sort_indices()
+    A = CSR(n, S.indptr.astype(np.int32), S.indices.astype(np.int32), S.data.astype(np.float64))
+    p = Problem("inv", A, b, np.zeros(n), m, 0.0, d, (fmt,), {})
+    ref = oracle.gmres(A, b, np.zeros(n), m, 0.0, d, fmt)
+    x, r = _solve_gpu(p, fmt, restart=m, rel_tol=0.0, max_iters=d, history=True)
+    assert ref.breakdown == 1 and ref.iters == d and ref.restarts == 1
+    assert r.breakdown == 1 and r.iters == d and r.restarts == 1 and r.reorth_count == ref.reorth_count == d
+    assert r.rel_res_recurrence > 0.0  # the cycle was not ended by hn == 0 or by the residual test
+    assert np.linalg.norm(x - xs) <= 50 * u * np.linalg.norm(xs) and not x[d:].any()
+    assert np.allclose(r.rec_history[: d - 1], ref.rec_history[: d - 1], rtol=1e-3)
+    # with a reachable tau: restart from the explicit residual, every cycle cut at step d, converged
+    p2 = Problem("inv", A, b, np.zeros(n), m, 1e-12, 200, (fmt,), {})
+    x2, r2 = _solve_gpu(p2, fmt)
+    ref2 = oracle.gmres(A, b, np.zeros(n), m, 1e-12, 200, fmt)
+    assert r2.converged and ref2.converged and r2.iters <= d * r2.restarts
+    assert abs(r2.iters - ref2.iters) <= d and np.linalg.norm(x2 - xs) <= 1e-10 * np.linalg.norm(xs)
+    # REORTH_NEVER has no such clause: the cycle runs on to m
+    _, r3 = _solve_gpu(p, fmt, restart=m, rel_tol=0.0, max_iters=m, reorth="never")
+    assert r3.iters == m and r3.breakdown == 0
+
+
+# ---- restart lengths beyond one launch's 128 columns (PAPER.md:294 sweeps m = 10 .. 300; NEXT-2) ------------------
+
+@pytest.mark.parametrize("m", [150, 300])
+@pytest.mark.parametrize("fmt", ["fp64", "fp32", "int16"])
+def test_long_restart_split_ranges_match_oracle(m, fmt):
+    """m > 128: every pass is split into ranges of <= 128 basis vectors and the fused update + multi-dot is
+    replaced by separate passes.  C2 on a 40^3 grid with tau = 1e-11 needs 140 steps with an fp64 basis (one
+    cycle) and 230 / 330-390 with fp32 / int16 (several cycles): iteration counts and residuals against the oracle."""
+    p = make_config("C2", grid=40)
+    r, ref = _check_parity(p, fmt, restart=m, rel_tol=1e-11, max_iters=3000, label=f"C2-40-m{m}")
+    assert r.converged and r.iters > 128  # the split path really ran
+    if fmt == "fp64":
+        assert r.reorth_count == ref.reorth_count
+
+
+@pytest.mark.parametrize("fmt", ["fp64", "int16"])
+def test_long_restart_whole_cycle_of_300_steps_matches_oracle(fmt):
+    """A whole cycle of m = 300 steps at a fixed iteration count (tau = 0, the protocol of PAPER.md:294): ranges of
+    128 + 128 + 44 vectors in every pass.  fp64 storage: the residual history equals the oracle's to rounding
+    while it is above 1e-10; int16: over the first 40 steps to the format's roundoff."""
+    p = make_config("C2", grid=40)
+    m = 300
+    ref = oracle.gmres(p.A, p.b, p.x0, m, 0.0, m, fmt)
+    x, r = _solve_gpu(p, fmt, restart=m, rel_tol=0.0, max_iters=m, history=True)
+    assert r.iters == ref.iters == m and r.restarts == ref.restarts == 1 and not r.converged
+    hg, ho = np.asarray(r.rec_history), np.asarray(ref.rec_history)
+    if fmt == "fp64":
+        live = ho > 1e-10
+        assert live.sum() > 128 and np.allclose(hg[live], ho[live], rtol=1e-8)
+        assert abs(r.reorth_count - ref.reorth_count) <= 2
+    else:
+        assert np.all(np.abs(hg[:40] - ho[:40]) <= 2.0 ** -15 * 4 * ho[:40])
+    tg, to = _true_rel_res(p, x), _true_rel_res(p, ref.x)
+    assert tg <= 10 * to and to <= 10 * tg
+
+
+# ---- the paper's protocol: b_i = sin(i), m = 100, tau = 1e-9, scalar Jacobi (PAPER.md:251, 186; NEXT-3) -----------
+
+@pytest.mark.parametrize("cfg,kw,label", [("C2", {"grid": 24}, "PP-C2-24"), ("C5", {"grid": 16}, "PP-C5-16"), ("C4", {"n": 20000}, "PP-C4-20k")])
+@pytest.mark.parametrize("fmt", oracle.FORMATS)
+def test_paper_protocol_small_matrices_match_oracle(cfg, kw, label, fmt):
+    from workloads import Problem
+
+    q = make_config(cfg, **kw)
+    n = q.A.n
+    b = np.sin(np.arange(1, n + 1, dtype=np.float64))
+    p = Problem(label, q.A, b, np.zeros(n), 100, 1e-9, 3000, oracle.FORMATS, {})
+    if label == "PP-C4-20k" and fmt in ("fp16", "int16"):
+        # 16-bit storage stagnates on the Jacobi-scaled power-law matrix (DESIGN.md 6.6): both sides stop at a
+        # short bound with comparable residuals instead of running thousands of chaotic steps
+        r, ref = _check_parity(p, fmt, max_iters=200, precond="jacobi", label=label)
+    else:
+        r, ref = _check_parity(p, fmt, precond="jacobi", label=label)
+        assert r.converged and ref.converged
+
+
+# ---- library hygiene: handles share no mutable state -----------------------------------------------------------
+
+def test_two_handles_with_different_options_do_not_interfere():
+    """Two handles on two streams with different pdl / orth_seg_kb / orth_interleave options, solves
+    interleaved: each result is bitwise the one the same handle gives alone."""
+    import torch
+    from paper_2009_12101_b200 import Solver
+
+    p = make_config("C2", grid=28)
+    opts = ({"pdl": 1, "orth_seg_kb": 0, "orth_interleave": 0}, {"pdl": 0, "orth_seg_kb": 1, "orth_interleave": 1})
+
+    def make(o, stream):
+        s = Solver(0, stream=stream)
+        for k, v in o.items():
+            s.set_option(k, v)
+        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+        return s
+
+    alone = []
+    for o in opts:
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            s = make(o, st)
+            x, r = s.solve(p.b, p.x0, 40, 1e-8, 400, "fp16", history=True)
+            st.synchronize()
+            alone.append((x.cpu().numpy(), r.rec_history.copy(), r.iters))
+            s.destroy()
+    st = [torch.cuda.Stream(), torch.cuda.Stream()]
+    hs = []
+    for o, t in zip(opts, st):
+        with torch.cuda.stream(t):
+            hs.append(make(o, t))
+    try:
+        for rep in range(2):
+            for i in (0, 1, 1, 0):
+                with torch.cuda.stream(st[i]):
+                    x, r = hs[i].solve(p.b, p.x0, 40, 1e-8, 400, "fp16", history=True)
+                    st[i].synchronize()
+                    assert r.iters == alone[i][2]
+                    assert np.array_equal(r.rec_history, alone[i][1])
+                    assert np.array_equal(x.cpu().numpy(), alone[i][0])
+    finally:
+        for s in hs:
+            s.destroy()
