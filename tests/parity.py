@@ -10,13 +10,16 @@ thread counts; nothing else about it changes).  So, for quantised formats only:
 
   * strict:  |gpu - oracle| <= max(2, 2 %)                                   -- always tried first;
   * band:    min(draws) - 2 % <= gpu <= max(draws) + 2 % over the oracle's own counts ("draws": the base run plus
-             the runs at other thread counts) -- used when the oracle's own draws differ by more than 2 %;
-  * chaotic: the band extended by two sample standard deviations of the draws -- ONLY for the (case, format)
-             pairs listed in CHAOTIC below, and only with at least MIN_DRAWS_FOR_SD draws.  These cases pin
+             the runs at other thread counts) -- for any quantised format whose oracle draws differ among themselves;
+  * chaotic: the band extended by two sample standard deviations of the draws -- ONLY for the 16-bit formats
+             (the paper's own Table 2 puts the variance of their iteration overhead at 62.3 / 46.95 against 0.01
+             for the 32-bit formats), only with at least MIN_DRAWS_FOR_SD draws (a further draw
+             falls outside the range of five with probability 1/3, so a range of few draws is no band), and never wider
+             than +-MAX_REL_HALF_WIDTH around the draws' median unless the case is listed in KNOWN_WIDE.  These cases pin
              nothing about kernel quality; tests/test_gpu_step_parity.py (teacher-forced single Arnoldi steps,
              where nothing is chaotic) is what discriminates there.
 
-Every use of a band is printed with all counts, so the test log shows which cases needed it.
+Every use of a band is printed with all counts, so the test log (-s) shows which cases needed which rule.
 """
 from __future__ import annotations
 
@@ -24,12 +27,15 @@ import numpy as np
 
 import oracle
 
-# (case label, format) pairs whose oracle draws are known to scatter by tens of per cent (Q11):
-# the Jacobi-preconditioned power-law matrix with 16-bit storage stagnates near tau for hundreds of steps.
-CHAOTIC = {("C4J-40k", "int16"), ("C4J-40k", "fp16"), ("C4B-40k", "int16"), ("C4B-40k", "fp16")}
+SIXTEEN_BIT = ("fp16", "int16")
 MIN_DRAWS_FOR_SD = 10
+MAX_REL_HALF_WIDTH = 0.15
+# (case label, format) pairs whose oracle draws scatter by tens of per cent (Q11): 16-bit storage on the
+# Jacobi- / block-Jacobi-preconditioned power-law matrix stagnates near tau for hundreds of steps (oracle draws
+# 731 .. 1125 for int16).  Only these may exceed MAX_REL_HALF_WIDTH.
+KNOWN_WIDE = {("C4J-40k", "int16"), ("C4B-40k", "int16")}
 SPREAD_THREADS = (1, 2, 3, 5)
-CHAOTIC_THREADS = (1, 2, 3, 4, 5, 6, 7, 9, 10, 11, 12)
+CHAOTIC_THREADS = (4, 6, 7, 9, 10, 11, 12)  # on top of SPREAD_THREADS: 12 draws with the base run
 
 
 def tol2(c: float) -> float:
@@ -70,13 +76,22 @@ def check_iters(gpu_iters: int, ref_iters: int, fmt: str, label: str, draws=None
     if strict_ok(gpu_iters, ref_iters):
         return "strict"
     assert fmt != "fp64", f"{label} fp64: gpu {gpu_iters} vs oracle {ref_iters}: fp64 storage has no quantisation, no band"
-    chaotic = (label, fmt) in CHAOTIC
     if draws is None:
         assert run is not None, f"{label} {fmt}: gpu {gpu_iters} vs oracle {ref_iters} and no oracle spread available"
-        draws = oracle_draws(run, CHAOTIC_THREADS if chaotic else SPREAD_THREADS)
+        draws = oracle_draws(run, SPREAD_THREADS)
     draws = [ref_iters] + list(draws)
-    lo, hi = band_of(draws, allow_sd=chaotic)
-    rule = "chaotic" if chaotic and len(draws) >= MIN_DRAWS_FOR_SD else "band"
-    print(f"[parity] {label} {fmt}: gpu {gpu_iters}, oracle draws {sorted(draws)} -> {rule} [{lo:.1f}, {hi:.1f}]")
-    assert lo <= gpu_iters <= hi, (label, fmt, gpu_iters, sorted(draws), rule)
-    return rule
+    lo, hi = band_of(draws, allow_sd=False)
+    if lo <= gpu_iters <= hi:
+        print(f"[parity] {label} {fmt}: gpu {gpu_iters}, oracle draws {sorted(draws)} -> band [{lo:.1f}, {hi:.1f}]")
+        return "band"
+    assert fmt in SIXTEEN_BIT, (label, fmt, gpu_iters, sorted(draws), "32-bit storage: no statistical band")
+    if len(draws) < MIN_DRAWS_FOR_SD and run is not None:
+        draws += oracle_draws(run, CHAOTIC_THREADS)
+    assert len(draws) >= MIN_DRAWS_FOR_SD, (label, fmt, gpu_iters, sorted(draws), "too few oracle draws for a statistical band")
+    lo, hi = band_of(draws, allow_sd=True)
+    med = float(np.median(draws))
+    if (label, fmt) not in KNOWN_WIDE:
+        lo, hi = max(lo, med * (1 - MAX_REL_HALF_WIDTH)), min(hi, med * (1 + MAX_REL_HALF_WIDTH))
+    print(f"[parity] {label} {fmt}: gpu {gpu_iters}, oracle draws {sorted(draws)} -> chaotic [{lo:.1f}, {hi:.1f}]")
+    assert lo <= gpu_iters <= hi, (label, fmt, gpu_iters, sorted(draws), "chaotic")
+    return "chaotic"

@@ -408,17 +408,17 @@ def test_long_restart_split_ranges_match_oracle(m, fmt):
 @pytest.mark.parametrize("fmt", ["fp64", "int16"])
 def test_long_restart_whole_cycle_of_300_steps_matches_oracle(fmt):
     """A whole cycle of m = 300 steps at a fixed iteration count (tau = 0, the protocol of PAPER.md:294): ranges of
-    128 + 128 + 44 vectors in every pass.  fp64 storage: the residual history equals the oracle's to rounding
-    while it is above 1e-10; int16: over the first 40 steps to the format's roundoff."""
-    p = make_config("C2", grid=40)
+    128 + 128 + 44 vectors in every pass.  2D Laplacian on a 128^2 grid (C1's recipe), which is still at a relative
+    residual of 8e-9 after 300 unrestarted steps.  fp64 storage: the residual history equals the oracle's to rounding
+    over the whole cycle; int16: over the first 40 steps to the format's roundoff."""
+    p = make_config("C1", grid=128)
     m = 300
     ref = oracle.gmres(p.A, p.b, p.x0, m, 0.0, m, fmt)
     x, r = _solve_gpu(p, fmt, restart=m, rel_tol=0.0, max_iters=m, history=True)
-    assert r.iters == ref.iters == m and r.restarts == ref.restarts == 1 and not r.converged
+    assert r.iters == m and ref.iters == m and r.restarts == 1 and ref.restarts == 1 and not r.converged
     hg, ho = np.asarray(r.rec_history), np.asarray(ref.rec_history)
     if fmt == "fp64":
-        live = ho > 1e-10
-        assert live.sum() > 128 and np.allclose(hg[live], ho[live], rtol=1e-8)
+        assert np.allclose(hg, ho, rtol=1e-8)
         assert abs(r.reorth_count - ref.reorth_count) <= 2
     else:
         assert np.all(np.abs(hg[:40] - ho[:40]) <= 2.0 ** -15 * 4 * ho[:40])
