@@ -318,6 +318,9 @@ def run_ours(args) -> int:
     p = _make_problem(args.workload)
     n, nnz = p.A.n, p.A.nnz
     solver = Solver(local)
+    for o in args.opt:
+        name, val = o.split("=")
+        solver.set_option(name, int(val))
     solver.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
     dev = {"b": torch.as_tensor(p.b, device=solver.device), "x0": torch.as_tensor(p.x0, device=solver.device)}
     host = {k: torch.as_tensor(v).pin_memory() for k, v in
@@ -460,7 +463,7 @@ def run_ours(args) -> int:
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": args.workload, "precond": PRECOND, "n": n, "nnz": nnz, "restart": p.restart, "rel_tol": p.rel_tol,
-                   "max_iters": p.max_iters, "formats": list(p.formats), "reorth": "cond (eta = 1/sqrt 2)",
+                   "max_iters": p.max_iters, "formats": list(p.formats), "reorth": "cond (eta = 1/sqrt 2)", "options": list(args.opt),
                    "step": "one solve to convergence per storage format",
                    "timed_region": "library event brackets off (profile = 0); roofline/kernels from a separate pass afterwards",
                    "l2": "no flush: the basis (0.8-3.3 GB on C5) + matrix (1.3 GB) exceed the 126 MB L2; reuse inside a solve is the workload's own",
@@ -490,6 +493,7 @@ def main() -> int:
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip per_config, c3 and msweep")
     ap.add_argument("--precond", choices=("none", "jacobi", "block_jacobi4"), default="none")
+    ap.add_argument("--opt", action="append", default=[], help="name=value for cbgmres_set_option (tuning experiments; repeatable)")
     args = ap.parse_args()
     global PRECOND
     PRECOND = args.precond

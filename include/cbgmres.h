@@ -151,6 +151,9 @@ const char *cbgmres_last_error(cbgmres_handle_t h);
  * cbgmres_profile_get; 1 = every step), default 0.  "pdl": 1 (default) = launch the step kernels with
  * programmatic stream serialisation (each parks in griddepcontrol.wait until its predecessor is done).
  * "orth_fuse": 1 (default) = fuse the first update with the second pass's multi-dot (one read of V).
+ * "orth_fused_rows": the fused pass maps warps to rows and adds the update's partial sums with shuffles
+ * (orth_fused_kernel) for 2 (default) = the 16-bit formats, 1 = every reduced format, 0 = never (the column-mapped
+ * kind of orth_kernel with its shared-memory reduction).
  * "orth_seg_kb": 0 (default, chosen per launch), 1, 2 or 4 = KB per column segment of the
  * Gram-Schmidt passes' row tiles.  "orth_interleave": 0 (default) or 2 = row tiles dealt round-robin to
  * the CTAs, 1 = one contiguous row range per CTA.  Every option belongs to the handle it is set on.

@@ -67,6 +67,7 @@ struct LaunchCtx {
     int device = 0;
     int use_pdl = 1;      // "pdl" option: programmatic dependent launch of the step kernels
     int interleave = 0;   // "orth_interleave" option: 0 auto, 1 blocked row ranges, 2 interleaved row tiles
+    int fused_rows = 2;   // "orth_fused_rows" option: row-mapped fused update + multi-dot: 0 never, 1 every reduced format, 2 (default) 16-bit formats
     int orth_error = 0;   // CUresult of a failed tensor-map encode (0 = none)
     cudaError_t launch_error = cudaSuccess; // first failed kernel launch since the last take_launch_error
     const char *launch_kernel = "";         // ... and which kernel it was

@@ -31,6 +31,7 @@
 // (deterministic, no fp64 atomics), applies the per-vector scales and takes the decisions of
 // Fig. 1 lines 7 and 12 on the device.
 #include <cuda.h> // CUtensorMap (types only; the encoder is fetched with cudaGetDriverEntryPoint)
+#include <type_traits>
 
 #include "device_utils.cuh"
 
@@ -813,6 +814,397 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
 }
 
 
+// ---- fused update + multi-dot for the reduced formats: warps own rows, lane groups own columns ---------------
+// The column-mapped fused kind above pays a k-INDEPENDENT price per row: the eight partial row vectors of a
+// tile go through shared memory (160 bytes of shared-memory traffic per row) between two CTA-wide barriers
+// that put all sixteen warps in lock-step -- measured (clock64 probes, n = 4.2e6, fp16): 40 % of a tile's time
+// is barrier / data wait, and the pass costs ~57 us more than its bytes at every k.  Here the 32 lanes of a
+// warp are 8 groups of 4: group j owns column 8 ch + j of every 8-column chunk, its four lanes own the 16-byte
+// payload words of the warp's rows (64 or 128 bytes of each column segment per warp).  The partial sums of
+// the update are then spread over the lane GROUPS of one warp and are added by a transposing butterfly of
+// shuffles -- no shared memory, no barrier, the sixteen warps drift apart and hide each other's latencies.
+// The new w leaves the lane that holds the finished row (global store + a per-warp shared buffer for the
+// second sweep, __syncwarp only); w itself is fetched from global memory into registers at the start of the
+// tile, so there is no w ring either.
+// Shared-memory layout of a chunk: the basis is seen as the 3D array [128-byte segments][columns][16 words]
+// and a TMA box [16 words x 8 columns x SEGS segments] lands as rows rho = 8 seg + col of 128 bytes with the
+// 128-byte swizzle (16-byte chunk index XOR rho mod 8 = col): the four lanes of each of the eight groups hit
+// all eight 16-byte bank groups four times per 512-byte wavefront set -- the minimum for a 128-bit warp load.
+constexpr int kFGroups = 8; // lane groups per warp = columns per chunk
+
+template <int FMT, int WPL> struct FTile {
+    using Fm = Fmt<FMT>;
+    static constexpr int VEC = Fm::VEC, B = Fm::BYTES;
+    static constexpr int SEGS = 8 * WPL;                 // 128-byte segments per column segment
+    static constexpr int SEG = SEGS * 128;               // 1 or 2 KB per column and tile
+    static constexpr int R = SEG / B;                    // rows of a tile
+    static constexpr int RW = R / kConsumerWarps;        // rows of a warp (64 * WPL bytes of every column)
+    static constexpr int NV = VEC * WPL;                 // rows of a lane
+    static constexpr int BOX_BYTES = kFGroups * SEG;     // one chunk of 8 columns: 8 or 16 KB
+    static constexpr int CPS = kStageBytes / BOX_BYTES;  // chunks per 32 KB stage: 4 or 2
+    static constexpr int STAGE_COLS = CPS * kFGroups;
+    static constexpr int W1_BYTES = R * 8;               // the new w of the tile, per-warp slices
+};
+__host__ __device__ constexpr int ffixed_smem(int R) { return 2048 + R * 8; } // barriers, coefficients, w1 (then 1 KB-aligned stages)
+
+__device__ __forceinline__ void tma_box3_g2s(void *dst_smem, const CUtensorMap *map, int x, int y, int z, uint64_t *bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+            smem_u32(dst_smem)),
+        "l"(map), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar))
+        : "memory");
+}
+
+// Transposing butterfly over the 8 lane groups (lane bits 4, 3, 2): every lane holds N partial sums (one per row
+// of its payload words, summed over the columns of ITS group); afterwards the lane holds max(1, N / 8) finished
+// sums, those with index fgroup_first<N>(lane) ... (for N < 8 both lanes of a pair hold the same sum).
+template <int N, int OFF, int NOUT> __device__ __forceinline__ void fgroup_reduce(double (&a)[N], int lane, double (&out)[NOUT])
+{
+    if constexpr (OFF < 4) {
+        static_assert(N == NOUT, "butterfly ends with NOUT sums per lane");
+#pragma unroll
+        for (int i = 0; i < N; ++i) out[i] = a[i];
+    } else if constexpr (N == 1) {
+        double b[1] = {a[0] + shfl_xor_f64(a[0], OFF)};
+        fgroup_reduce<1, OFF / 2, NOUT>(b, lane, out);
+    } else {
+        constexpr int H = N / 2;
+        const bool up = (lane & OFF) != 0;
+        double b[H];
+#pragma unroll
+        for (int i = 0; i < H; ++i) {
+            const double send = up ? a[i] : a[i + H];
+            const double keep = up ? a[i + H] : a[i];
+            b[i] = keep + shfl_xor_f64(send, OFF);
+        }
+        fgroup_reduce<H, OFF / 2, NOUT>(b, lane, out);
+    }
+}
+// index (into the lane's N rows) of the first finished sum a lane holds after fgroup_reduce<N, 16>
+template <int N> __device__ __forceinline__ int fgroup_first(int lane)
+{
+    int idx = 0, n = N;
+#pragma unroll
+    for (int off = 16; off >= 4; off >>= 1) {
+        if (n > 1) {
+            n >>= 1;
+            if (lane & off) idx += n;
+        }
+    }
+    return idx;
+}
+
+template <int FMT, int WPL>
+__global__ void __launch_bounds__(kOrthThreads, 1)
+    orth_fused_kernel(const OrthArgs a, const __grid_constant__ CUtensorMap tmap)
+{
+    using T = FTile<FMT, WPL>;
+    using Fm = typename T::Fm;
+    constexpr int VEC = T::VEC, B = T::B, R = T::R, NV = T::NV, RW = T::RW;
+    constexpr int NOUT = NV >= 8 ? NV / 8 : 1; // finished rows per lane after the butterfly
+    constexpr double PRE = Fm::PRE;
+    Ctl *ctl = a.ctl;
+    const int ns = a.nstages;
+
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u); // the swizzle pattern repeats every 1 KB
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem);
+    uint64_t *empty = full + kMaxStages;
+    double *hs_s = reinterpret_cast<double *>(smem + 1024);
+    double *w1 = reinterpret_cast<double *>(smem + 2048);
+    unsigned char *stages = smem + ((ffixed_smem(R) + 1023) & ~1023);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        for (int s = 0; s < ns; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], kConsumerWarps);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // row tiles dealt round-robin to the CTAs (the CTAs sweep a contiguous window of the basis together)
+    const int64_t total = (a.n + R - 1) / R;
+    int ntiles = (int)((total - blockIdx.x + gridDim.x - 1) / gridDim.x);
+    if (ntiles < 0) ntiles = 0;
+    const int64_t row_begin = (int64_t)blockIdx.x * R, tile_stride = (int64_t)gridDim.x * R;
+    const int dir = a.dir;
+
+    auto issue_stage = [&](int64_t r0, int st, int slot, int kk) { // lanes 0..CPS-1 issue one chunk each
+        const int c_first = st * T::STAGE_COLS;
+        const int nboxes = min(T::CPS, (kk - c_first + kFGroups - 1) / kFGroups);
+        if (lane == 0) mbar_expect_tx(&full[slot], nboxes * T::BOX_BYTES);
+        __syncwarp();
+        if (lane < nboxes)
+            tma_box3_g2s(stages + (size_t)slot * kStageBytes + lane * T::BOX_BYTES, &tmap, 0, c_first + lane * kFGroups,
+                         (int)(r0 * B / 128), &full[slot]);
+    };
+
+    // the basis is not written by the predecessor kernel: first stages before the grid dependency resolves
+    int pre = 0;
+    if (warp == kConsumerWarps && ntiles > 0) {
+        const int nst0 = (a.k + T::STAGE_COLS - 1) / T::STAGE_COLS;
+        pre = nst0 < ns ? nst0 : ns;
+        const int t0 = dir ? ntiles - 1 : 0;
+        for (int st = 0; st < pre; ++st) issue_stage(row_begin + (int64_t)t0 * tile_stride, st, st, a.k);
+    }
+    pdl_wait();
+    pdl_launch_dependents();
+    const int stop_after = __ldcg(&ctl->stop_after);
+    double hs_v = 0.0;
+    if (tid < a.k) hs_v = __ldcg(&a.hs[tid]);
+    const int k = a.k;
+    if (a.mode == MODE_ORTH1 && a.step > stop_after) { // copies in flight must land before the CTA gives its shared memory back
+        if (warp == kConsumerWarps && lane == 0)
+            for (int s = 0; s < pre; ++s) mbar_wait(&full[s], 0u);
+        return;
+    }
+    const int nst = (k + T::STAGE_COLS - 1) / T::STAGE_COLS;
+    if (tid < kConsumers) {
+        if (tid < kMaxRangeCols) hs_s[tid] = (tid < k) ? hs_v * PRE : 0.0;
+        consumer_bar();
+    }
+
+    double acc[kMaxChunks];
+#pragma unroll
+    for (int i = 0; i < kMaxChunks; ++i) acc[i] = 0.0;
+    double ss = 0.0, am = 0.0;
+
+    if (warp == kConsumerWarps) {
+        // ---- producer --------------------------------------------------------------------------------------
+        Ring ring;
+        for (int i = 0; i < ntiles; ++i) {
+            const int t = dir ? ntiles - 1 - i : i;
+            const int64_t r0 = row_begin + (int64_t)t * tile_stride;
+            for (int st = 0; st < nst; ++st) {
+                if (i > 0 || st >= pre) {
+                    if (lane == 0) mbar_wait(&empty[ring.s], ring.ph ^ 1u);
+                    issue_stage(r0, st, ring.s, k);
+                }
+                ring.advance(ns);
+            }
+        }
+    } else {
+        // ---- consumers: warp w owns rows [w RW, (w+1) RW) of every tile; lane = (group j, word t) -----------
+        const int j = lane >> 2, t4 = lane & 3;
+        // byte offset of this lane's word(s) inside a chunk: row rho = 8 seg + j of 128 bytes, 16-byte chunk c ^ j
+        int woff[WPL], rloc[WPL]; // ... and the first row (within the warp's rows) each word covers
+        if constexpr (WPL == 1) {
+            const int seg = warp >> 1, c = 4 * (warp & 1) + t4;
+            woff[0] = (seg * 8 + j) * 128 + ((c ^ j) & 7) * 16;
+            rloc[0] = t4 * VEC;
+        } else {
+#pragma unroll
+            for (int q = 0; q < WPL; ++q) {
+                const int c = t4 + 4 * q;
+                woff[q] = (warp * 8 + j) * 128 + ((c ^ j) & 7) * 16;
+                rloc[q] = c * VEC;
+            }
+        }
+        double *w1w = w1 + warp * RW; // this warp's slice of the new w
+        const int ofirst = fgroup_first<NV>(lane); // index among the lane's NV rows of the row(s) it finishes
+        // rows (within the warp) this lane finishes: NV rows are ordered word 0 rows, word 1 rows
+        const int fin_r = rloc[ofirst / VEC] + (ofirst % VEC);
+        const bool fin_owner = NV >= 8 || (lane & (NV == 4 ? 4 : 12)) == 0; // for N < 8 several lanes hold the same sum: one writes
+        Ring ring;
+        for (int i = 0; i < ntiles; ++i) {
+            const int t = dir ? ntiles - 1 - i : i;
+            const int64_t r0 = row_begin + (int64_t)t * tile_stride;
+            const int64_t rows_left = a.n - r0; // rows of the tile that exist (may exceed R)
+            // the tile body, compiled twice: RAGGED = the tile runs past row n (masks per entry), else no masks
+            auto tile = [&](auto ragged_tag) {
+            constexpr bool ragged = decltype(ragged_tag)::value;
+            const int64_t gr = r0 + warp * RW + fin_r; // global row of the first row this lane finishes
+            // old w of the rows this lane will finish: in flight during the first sweep
+            double wold[NOUT];
+#pragma unroll
+            for (int e = 0; e < NOUT; ++e) wold[e] = 0.0;
+            if (fin_owner) {
+                if (NOUT == 2 && gr + 1 < a.n) {
+                    const double2 v2 = __ldcg(reinterpret_cast<const double2 *>(a.w + gr));
+                    wold[0] = v2.x;
+                    wold[NOUT - 1] = v2.y;
+                } else {
+#pragma unroll
+                    for (int e = 0; e < NOUT; ++e)
+                        if (gr + e < a.n) wold[e] = __ldcg(a.w + gr + e);
+                }
+            }
+            // rows of this lane's words that exist (ragged tile): word q covers warp rows rloc[q] .. rloc[q] + VEC
+            int live[WPL];
+#pragma unroll
+            for (int q = 0; q < WPL; ++q) {
+                const int64_t left = rows_left - (warp * RW + rloc[q]);
+                live[q] = ragged ? (int)max((int64_t)0, min((int64_t)VEC, left)) : VEC;
+            }
+            const Ring tile_start = ring;
+            // ---- sweep 1: p = sum over this group's columns of dec(V)[rows, c] * hs_c ---------------------------
+            double p[NV];
+#pragma unroll
+            for (int v = 0; v < NV; ++v) p[v] = 0.0;
+            for (int st = 0; st < nst; ++st) {
+                mbar_wait(&full[ring.s], ring.ph);
+                const unsigned char *stg = stages + (size_t)ring.s * kStageBytes;
+                const int nch = min(T::CPS, (k - st * T::STAGE_COLS + kFGroups - 1) / kFGroups); // chunks with a wanted column
+                // NC = chunks of this stage that hold a wanted column (CPS for every stage but a tile's last):
+                // all loads first, then the NC * WPL independent decode + FMA chains
+                auto chunks = [&](auto nc_tag) {
+                    constexpr int NC = decltype(nc_tag)::value;
+                    uint4 raw[NC][WPL];
+                    double coef[NC];
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) {
+                        coef[c] = hs_s[st * T::STAGE_COLS + c * kFGroups + j]; // zero beyond k
+#pragma unroll
+                        for (int q = 0; q < WPL; ++q)
+                            raw[c][q] = (live[q] > 0) ? *reinterpret_cast<const uint4 *>(stg + c * T::BOX_BYTES + woff[q])
+                                                      : make_uint4(0u, 0u, 0u, 0u);
+                    }
+#pragma unroll
+                    for (int c = 0; c < NC; ++c)
+#pragma unroll
+                        for (int q = 0; q < WPL; ++q) {
+                            double d[VEC];
+                            Fm::decode(raw[c][q], d);
+#pragma unroll
+                            for (int v = 0; v < VEC; ++v) {
+                                if (ragged && v >= live[q]) d[v] = 0.0; // padding beyond n may decode to anything
+                                p[q * VEC + v] = fma(d[v], coef[c], p[q * VEC + v]);
+                            }
+                        }
+                };
+                if (nch >= T::CPS) chunks(std::integral_constant<int, T::CPS>{});
+                else if (nch == 1) chunks(std::integral_constant<int, 1>{});
+                else if constexpr (T::CPS == 4) {
+                    if (nch == 2) chunks(std::integral_constant<int, 2>{});
+                    else chunks(std::integral_constant<int, 3>{});
+                }
+                ring.advance(ns);
+            }
+            // ---- the partial sums of the 8 groups -> finished rows; new w ---------------------------------------
+            double tot[NOUT];
+            fgroup_reduce<NV, 16, NOUT>(p, lane, tot);
+            double wn[NOUT];
+#pragma unroll
+            for (int e = 0; e < NOUT; ++e) {
+                wn[e] = (PRE == 1.0) ? wold[e] - tot[e] : fma(-tot[e], PRE, wold[e]); // tot * PRE is exact: one rounding either way
+                const bool exists = gr + e < a.n;
+                if (!exists) wn[e] = 0.0;
+                if (fin_owner && exists) {
+                    ss = fma(wn[e], wn[e], ss);
+                    am = fmax(am, fabs(wn[e]));
+                }
+            }
+            if (fin_owner) {
+                if (NOUT == 2) {
+                    *reinterpret_cast<double2 *>(w1w + fin_r) = make_double2(wn[0], wn[NOUT - 1]);
+                    if (gr + 1 < a.n) *reinterpret_cast<double2 *>(a.w + gr) = make_double2(wn[0], wn[NOUT - 1]);
+                    else if (gr < a.n) a.w[gr] = wn[0];
+                } else {
+                    w1w[fin_r] = wn[0];
+                    if (gr < a.n) a.w[gr] = wn[0];
+                }
+            }
+            __syncwarp();
+            // ---- sweep 2 over the resident chunks: u_c += sum_rows dec(V)[r, c] * w_new[r] ----------------------
+            double wreg[NV];
+#pragma unroll
+            for (int q = 0; q < WPL; ++q)
+#pragma unroll
+                for (int v = 0; v < VEC; v += 2) {
+                    const double2 t2 = *reinterpret_cast<const double2 *>(w1w + rloc[q] + v);
+                    wreg[q * VEC + v] = (PRE == 1.0) ? t2.x : t2.x * PRE;
+                    wreg[q * VEC + v + 1] = (PRE == 1.0) ? t2.y : t2.y * PRE;
+                }
+            __syncwarp(); // w1w is rewritten by the next tile only after every lane has read it
+            Ring r2 = tile_start;
+#pragma unroll
+            for (int st = 0; st < kMaxChunks / T::CPS; ++st) {
+                if (st < nst) {
+                    const unsigned char *stg = stages + (size_t)r2.s * kStageBytes;
+                    const int nch = min(T::CPS, (k - st * T::STAGE_COLS + kFGroups - 1) / kFGroups);
+                    auto chunks = [&](auto nc_tag) {
+                        constexpr int NC = decltype(nc_tag)::value;
+                        uint4 raw[NC][WPL];
+#pragma unroll
+                        for (int c = 0; c < NC; ++c)
+#pragma unroll
+                            for (int q = 0; q < WPL; ++q)
+                                raw[c][q] = (live[q] > 0) ? *reinterpret_cast<const uint4 *>(stg + c * T::BOX_BYTES + woff[q])
+                                                          : make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+                        for (int c = 0; c < NC; ++c)
+#pragma unroll
+                            for (int q = 0; q < WPL; ++q) {
+                                double d[VEC];
+                                Fm::decode(raw[c][q], d);
+                                if (ragged) {
+#pragma unroll
+                                    for (int v = 0; v < VEC; ++v)
+                                        if (v >= live[q]) d[v] = 0.0;
+                                }
+                                acc[st * T::CPS + c] += word_dot<VEC>(d, &wreg[q * VEC]);
+                            }
+                    };
+                    if (nch >= T::CPS) chunks(std::integral_constant<int, T::CPS>{});
+                    else if (nch == 1) chunks(std::integral_constant<int, 1>{});
+                    else if constexpr (T::CPS == 4) {
+                        if (nch == 2) chunks(std::integral_constant<int, 2>{});
+                        else chunks(std::integral_constant<int, 3>{});
+                    }
+                    unsigned dep = 0; // the sums have consumed every word loaded from the stage
+#pragma unroll
+                    for (int c = 0; c < T::CPS; ++c) dep ^= dep_bits(acc[st * T::CPS + c]);
+                    mbar_arrive_after_use(&empty[r2.s], lane, dep);
+                    r2.advance(ns);
+                }
+            }
+            };
+            if (rows_left < R) tile(std::true_type{});
+            else tile(std::false_type{});
+        }
+    }
+    // ---- CTA partials: the four lanes of a group, then the sixteen warps in a fixed order ----------------------
+    __syncthreads(); // every stage has been consumed: the stage memory is free for the partials
+    double *hpart = reinterpret_cast<double *>(stages);                       // [16 warps][128 columns]
+    double *npart_s = hpart + kConsumerWarps * kMaxRangeCols;                 // [2][16 warps]
+    if (warp < kConsumerWarps) {
+#pragma unroll
+        for (int ch = 0; ch < kMaxChunks; ++ch) {
+            double v = acc[ch];
+            v += shfl_xor_f64(v, 1);
+            v += shfl_xor_f64(v, 2);
+            if ((lane & 3) == 0) hpart[warp * kMaxRangeCols + ch * kFGroups + (lane >> 2)] = v * PRE; // acc holds sums / PRE
+        }
+        ss = warp_sum(ss);
+        am = warp_max(am);
+        if (lane == 0) {
+            npart_s[warp] = ss;
+            npart_s[kConsumerWarps + warp] = am;
+        }
+    }
+    __syncthreads();
+    for (int col = tid; col < k; col += kOrthThreads) {
+        double tsum = 0.0;
+#pragma unroll
+        for (int w = 0; w < kConsumerWarps; ++w) tsum += hpart[w * kMaxRangeCols + col];
+        a.partials[(size_t)blockIdx.x * kLdp + col] = tsum;
+    }
+    if (tid == 0) {
+        double tsum = 0.0, m = 0.0;
+        for (int w = 0; w < kConsumerWarps; ++w) {
+            tsum += npart_s[w];
+            m = fmax(m, npart_s[kConsumerWarps + w]);
+        }
+        a.npart[blockIdx.x] = tsum;
+        a.npart[kMaxGrid + blockIdx.x] = m;
+    }
+    if (!last_block_done(&ctl->tickets[0])) return;
+    orth_finalize<PASS_UPD_DOT, Fm::SCALED>(a, k, reinterpret_cast<double *>(stages) + 4096); // scratch after the partials (32 KB in)
+}
+
 // ---- few vectors (k <= 8): no staging --------------------------------------------------------------------
 // With at most eight basis vectors a row tile is a few KB and the staged kernel is bound by its
 // per-tile round trips (multi-dot, n = 4.2e6: 50 us for k = 1..4, whatever the format).  Here a thread
@@ -1111,6 +1503,95 @@ const CUtensorMap *w_map(LaunchCtx *lc, const double *w, int64_t n, int vec, int
     return &e.map;
 }
 
+// The basis as the 3D array [ceil(n*B/128) segments of 128 bytes][k columns][16 words of 8 bytes] for
+// orth_fused_kernel: box [16 x 8 columns x segs segments] with the 128-byte swizzle.  Needs ld*B % 128 == 0: the
+// last, partial segment of a column then reads that column's own padding (masked by the kernel).
+const CUtensorMap *basis_map3(LaunchCtx *lc, const void *V, int64_t ld, int64_t n, int bytes, int k, int segs)
+{
+    struct Entry {
+        MapKey key;
+        CUtensorMap map;
+    };
+    static thread_local Entry cache[2][kMaxRangeCols + 1];
+    Entry &e = cache[segs == 8 ? 0 : 1][k];
+    const MapKey key{V, ld, n, bytes, k, segs};
+    if (e.key == key) return &e.map;
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) {
+        lc->orth_error = 999;
+        return nullptr;
+    }
+    const cuuint64_t dims[3] = {16, (cuuint64_t)k, (cuuint64_t)((n * bytes + 127) / 128)};
+    const cuuint64_t strides[2] = {(cuuint64_t)(ld * bytes), 128};
+    const cuuint32_t box[3] = {16, (cuuint32_t)kFGroups, (cuuint32_t)segs};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult rc = fn(&e.map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 3, const_cast<void *>(V), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (rc != CUDA_SUCCESS) {
+        lc->orth_error = (int)rc;
+        e.key = MapKey{};
+        return nullptr;
+    }
+    e.key = key;
+    return &e.map;
+}
+
+inline int fused_stages(int format, int wpl)
+{
+    const int R = wpl * 1024 / fmt_bytes(format);
+    const int ns = (kOrthSmemBytes - 1024 - ((ffixed_smem(R) + 1023) & ~1023)) / kStageBytes;
+    return ns > kMaxStages ? kMaxStages : ns;
+}
+// words per lane and column (1 or 2, i.e. 1 or 2 KB column segments) for the row-mapped fused pass; 0 = not usable
+int choose_fused_wpl(int format, int k, int64_t n, int64_t ld, int forced_seg_kb)
+{
+    const int B = fmt_bytes(format);
+    if (B == 8 || k < 1 || k > kMaxRangeCols || (ld * B) % 128 != 0 || forced_seg_kb > 2) return 0;
+    const int64_t per = ((n + kNumSMs - 1) / kNumSMs + 63) / 64 * 64;
+    for (int wpl = 2; wpl >= 1; --wpl) {
+        if (forced_seg_kb && wpl != forced_seg_kb) continue;
+        if (wpl == 2 && B == 2 && !forced_seg_kb) continue; // 16 rows per lane: 96 registers do not hold them (spills)
+        const int nst = (k * wpl + 31) / 32; // a stage holds 32 / wpl columns
+        if (fused_stages(format, wpl) < nst + 1) continue;
+        if (wpl == 1 || forced_seg_kb || (int64_t)wpl * 1024 / B * 12 <= per) return wpl; // at least twelve row tiles per CTA
+    }
+    return 0;
+}
+
+template <int FMT, int WPL> int launch_fused_inst(cudaStream_t s, const Scratch &sc, OrthArgs &a)
+{
+    using T = FTile<FMT, WPL>;
+    static unsigned long long attr_set = 0;
+    if (first_use_on_device(attr_set, sc.lc->device))
+        cudaFuncSetAttribute(orth_fused_kernel<FMT, WPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, kOrthSmemBytes);
+    const CUtensorMap *map = basis_map3(sc.lc, a.V, a.ld, a.n, T::B, a.k, T::SEGS);
+    if (!map) return 0;
+    a.nstages = fused_stages(FMT, WPL);
+    a.interleave = 1;
+    int64_t grid = (a.n + T::R - 1) / T::R;
+    if (grid > kNumSMs) grid = kNumSMs;
+    const size_t smem = 1024 + (size_t)((ffixed_smem(T::R) + 1023) & ~1023) + (size_t)a.nstages * kStageBytes;
+    launch_chain(sc, "orth_fused_kernel", orth_fused_kernel<FMT, WPL>, dim3((unsigned)grid), dim3(kOrthThreads), smem, s, a, *map);
+    return 1;
+}
+
+template <int FMT> int launch_fused_f(cudaStream_t s, const Scratch &sc, OrthArgs &a, int wpl)
+{
+    return wpl == 2 ? launch_fused_inst<FMT, 2>(s, sc, a) : launch_fused_inst<FMT, 1>(s, sc, a);
+}
+
+int launch_fused(cudaStream_t s, const Scratch &sc, int format, OrthArgs &a, int wpl)
+{
+    switch (format) {
+    case CBGMRES_FP32: return launch_fused_f<CBGMRES_FP32>(s, sc, a, wpl);
+    case CBGMRES_FP16: return launch_fused_f<CBGMRES_FP16>(s, sc, a, wpl);
+    case CBGMRES_INT32: return launch_fused_f<CBGMRES_INT32>(s, sc, a, wpl);
+    case CBGMRES_INT16: return launch_fused_f<CBGMRES_INT16>(s, sc, a, wpl);
+    default: return 0;
+    }
+}
+
 template <int FMT, int F, int KIND> int launch_inst(cudaStream_t s, const Scratch &sc, OrthArgs &a)
 {
     using T = Tile<FMT, F>;
@@ -1263,6 +1744,13 @@ int launch_update_multidot(cudaStream_t s, const Scratch &sc, const BasisView &b
     a.h_out = h_out;
     a.hs_out = hs_out;
     if (use_small(a, b.format, seg_kb)) return launch_small<PASS_UPD_DOT>(s, sc, b.format, a);
+    // warps own rows, shuffle reduction (orth_fused_kernel): measured equal to the column-mapped kind within 1-3 % at every
+    // k (n = 4.2e6: fp16 k = 32 / 64 / 128: 124 / 192 / 290 us against 130 / 177 / 294; fp32 136 / 222 / 396 against 145 / 224 / 380),
+    // a little ahead for the 16-bit formats inside the solves (C2 int16 53 against 57 us), a little behind for the 32-bit ones
+    if (sc.lc->fused_rows == 1 || (sc.lc->fused_rows == 2 && fmt_bytes(b.format) == 2)) {
+        const int wpl = choose_fused_wpl(b.format, k, n, b.ld, seg_kb);
+        if (wpl) return launch_fused(s, sc, b.format, a, wpl);
+    }
     return launch_fmt<PASS_UPD_DOT>(s, sc, b.format, a, choose_seg_kb(b.format, PASS_UPD_DOT, k, n, seg_kb));
 }
 

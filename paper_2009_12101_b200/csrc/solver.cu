@@ -373,6 +373,11 @@ int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value)
         h->opt_fuse = value != 0;
         return CBGMRES_OK;
     }
+    if (!strcmp(name, "orth_fused_rows")) {
+        if (value < 0 || value > 2) return fail(h, CBGMRES_E_INVALID, "orth_fused_rows must be 0, 1 or 2");
+        h->lc.fused_rows = (int)value;
+        return CBGMRES_OK;
+    }
     if (!strcmp(name, "pdl")) {
         h->lc.use_pdl = value != 0;
         return CBGMRES_OK;

@@ -95,6 +95,7 @@ def main(argv=None) -> int:
     ap.add_argument("--interleave", type=int, default=0, help="orth_interleave option: 0 auto, 1 blocked, 2 interleaved")
     ap.add_argument("--spmv-kernel", default="0", help="comma list of spmv_kernel options to time (0 = auto)")
     ap.add_argument("--seg-kb", type=int, default=0, help="orth_seg_kb option: 0 auto, 1, 2, 4")
+    ap.add_argument("--opt", action="append", default=[], help="name=value, passed to cbgmres_set_option (repeatable)")
     args = ap.parse_args(argv)
     ks = [int(x) for x in args.k.split(",") if x]
     fmts = [f for f in args.formats.split(",") if f]
@@ -102,6 +103,9 @@ def main(argv=None) -> int:
     s = Solver(0)
     s.set_option("orth_seg_kb", args.seg_kb)
     s.set_option("orth_interleave", args.interleave)
+    for o in args.opt:
+        name, val = o.split("=")
+        s.set_option(name, int(val))
     dev = s.device
     out = run(s, n, ks, fmts, args.reps, args.flush) if ks and fmts else []
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev) if args.flush else None

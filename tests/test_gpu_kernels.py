@@ -228,6 +228,48 @@ def test_update_multidot_fused_matches_oracle(solver, fmt, n, k):
     assert np.all(np.abs(u_gpu - u_ref) <= 2 * TOL * Vhat_norm * scale)
 
 
+@pytest.mark.parametrize("fmt", ["fp32", "fp16", "int32", "int16"])
+@pytest.mark.parametrize("rows_mapped,seg_kb", [(1, 0), (1, 1), (1, 2), (0, 0)])
+@pytest.mark.parametrize("n,k,ld_extra", [(9, 9, 64), (1000, 9, 64), (40000, 17, 64), (70001, 128, 64), (200003, 33, 64),
+                                          (300000, 100, 0), (148 * 1024 * 3 + 5, 12, 64), (70001, 50, 8)])
+def test_fused_pass_both_mappings(fmt, rows_mapped, seg_kb, n, k, ld_extra):
+    """The fused update + multi-dot of the reduced formats in both mappings: warps own rows with a shuffle reduction
+    (orth_fused_kernel, 1 or 2 KB column segments: option orth_fused_rows = 1) and the column-mapped kind of
+    orth_kernel (= 0, also the fall-back when a column's stride is not a multiple of 128 bytes: ld_extra = 8).
+    Ragged last tiles, odd n, NaN-poisoned padding, k up to the 128 columns of one launch."""
+    import torch
+
+    from paper_2009_12101_b200 import Solver
+
+    s = Solver(0)
+    try:
+        s.set_option("orth_fused_rows", rows_mapped)
+        s.set_option("orth_seg_kb", seg_kb)
+        P, sig, w, dP, dsig = _basis(fmt, n, k, seed=480 + n + k, ld_extra=ld_extra)
+        h = np.random.default_rng(481).standard_normal(k)
+        w_ref, ss_ref, am_ref = oracle.ref_update(fmt, P[:k], sig[:k], h, w)
+        u_ref = oracle.ref_multidot(fmt, P, sig, w_ref, k=k)
+        dw = _dev(w).clone()
+        u, out = s.k_update_multidot(fmt, dP[:k], dsig[:k], _dev(h), dw, n=n)
+        torch.cuda.synchronize()
+        w_gpu, u_gpu = dw.cpu().numpy(), u.cpu().numpy()
+        nrm2, amax = out.cpu().numpy()
+        scale = np.linalg.norm(w) + np.linalg.norm(h)
+        Vhat_norm = np.array([np.linalg.norm(oracle.dec(fmt, P[c, :n], sig[c])) for c in range(k)])
+        assert np.linalg.norm(w_gpu - w_ref) <= TOL * scale
+        assert abs(nrm2 - np.sqrt(ss_ref)) <= TOL * scale
+        assert amax == np.abs(w_gpu).max()
+        assert np.all(np.isfinite(u_gpu))
+        assert np.all(np.abs(u_gpu - u_ref) <= 2 * TOL * Vhat_norm * scale)
+        # bitwise repeatable (fixed summation order)
+        dw2 = _dev(w).clone()
+        u2, out2 = s.k_update_multidot(fmt, dP[:k], dsig[:k], _dev(h), dw2, n=n)
+        torch.cuda.synchronize()
+        assert torch.equal(dw, dw2) and torch.equal(u, u2) and torch.equal(out, out2)
+    finally:
+        s.destroy()
+
+
 @pytest.mark.parametrize("fmt", FORMATS)
 @pytest.mark.parametrize("seg_kb", [1, 2, 4])
 @pytest.mark.parametrize("n,k", [(148 * 64 + 1, 5), (31111, 40), (70001, 129), (131072, 16)])
