@@ -14,7 +14,7 @@ from dataclasses import dataclass
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libcbgmres.so")
+LIB_PATH = os.environ.get("CBGMRES_LIB") or os.path.join(HERE, "libcbgmres.so")  # CBGMRES_LIB: another build of the same ABI
 
 FORMATS = ("fp64", "fp32", "fp16", "int32", "int16")
 FORMAT_CODE = {f: i for i, f in enumerate(FORMATS)}

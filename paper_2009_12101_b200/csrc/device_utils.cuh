@@ -30,7 +30,7 @@ __device__ __forceinline__ uint4 ldg_stream128(const void *p)
 // binade of 2^52; one fp64 subtraction removes the offset.
 // (Define CBG_DECODE_CVT to get the plain conversions back.)
 #ifdef CBG_DECODE_CVT
-constexpr double kPreF32 = 1.0, kPreF16 = 1.0;
+constexpr double kPreF32 = 1.0, kPreF16 = 1.0, kPreF16Even = 1.0;
 __device__ __forceinline__ double f32_bits_to_raw(unsigned f) { return (double)__uint_as_float(f); }
 __device__ __forceinline__ double i32_to_double(int q) { return (double)q; }
 // F2F.F64.F16 / I2F.F64.S16 take either half of a 32-bit register: one instruction per entry
@@ -55,6 +55,33 @@ __device__ __forceinline__ double i32_to_double(int q)
 {
     return __hiloint2double(0x43300000, q ^ (int)0x80000000) - 4503601774854144.0;
 }
+// Two 16-bit entries per 32-bit payload word, MIXED widening (CBG_DECODE_MIXED, default): the LOW half goes
+// through the conversion pipe (F2F.F64.F16 / I2F.F64.S16 read either half of a register: one instruction,
+// 16 per clock and SM), the HIGH half through the integer pipes (arithmetic shift + mask in place, no
+// left shift needed).  A 16-bit pass at the HBM rate delivers 11.2 entries per clock and SM: all of them
+// through the conversion pipe would saturate it, all of them through the integer pipes cost 3.8 issue
+// slots per entry (measured from ncu's instruction counts); half and half is 2.75.  For binary16 the two
+// halves then carry different powers of two -- the low half is the true value, the high half value * 2^-1008
+// -- so the OTHER operand of every product carries 2^-504 on even rows and 2^+504 on odd rows
+// (Fmt::PRE_EVEN / Fmt::PRE): every product is value * operand * 2^-504 exactly as before, bit for bit.
+#ifndef CBG_DECODE_MIXED
+#define CBG_DECODE_MIXED 1
+#endif
+#if CBG_DECODE_MIXED
+constexpr double kPreF16Even = 0x1p-504;
+__device__ __forceinline__ void half2_to_raw(unsigned w, double &lo, double &hi)
+{
+    asm("{.reg .b16 l, h; mov.b32 {l, h}, %1; cvt.f64.f16 %0, l;}" : "=d"(lo) : "r"(w));
+    const unsigned h1 = (unsigned)((int)w >> 6) & 0x81FFFC00u;
+    hi = __hiloint2double((int)h1, 0);
+}
+__device__ __forceinline__ void i16x2_to_doubles(unsigned w, double &lo, double &hi)
+{
+    asm("{.reg .b16 l, h; mov.b32 {l, h}, %1; cvt.rn.f64.s16 %0, l;}" : "=d"(lo) : "r"(w));
+    hi = __hiloint2double(0x43300000, (int)((w >> 16) ^ 0x8000u)) - 4503599627403264.0; // 2^52 + 32768 + q, minus the offset
+}
+#else
+constexpr double kPreF16Even = kPreF16;
 // two binary16 -> values * 2^-1008.
 __device__ __forceinline__ void half2_to_raw(unsigned w, double &lo, double &hi)
 {
@@ -72,6 +99,7 @@ __device__ __forceinline__ void i16x2_to_doubles(unsigned w, double &lo, double 
     hi = __hiloint2double(0x43300000, (int)(u >> 16)) - 4503599627403264.0;
 }
 #endif
+#endif
 
 // ---- storage formats ----------------------------------------------------------
 // VEC = entries per 128-bit load.  decode() widens one 128-bit payload word to VEC fp64 values
@@ -84,6 +112,7 @@ template <> struct Fmt<CBGMRES_FP64> {
     static constexpr int VEC = 2, BYTES = 8;
     static constexpr bool SCALED = false;
     static constexpr double PRE = 1.0; // decode() yields value / PRE^2 (see "widening" above)
+    static constexpr double PRE_EVEN = 1.0; // ... on even entries value / (PRE * PRE_EVEN) (mixed widening of binary16)
     __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
     {
         d[0] = __hiloint2double((int)r.y, (int)r.x);
@@ -96,6 +125,7 @@ template <> struct Fmt<CBGMRES_FP32> {
     static constexpr int VEC = 4, BYTES = 4;
     static constexpr bool SCALED = false;
     static constexpr double PRE = kPreF32;
+    static constexpr double PRE_EVEN = kPreF32; // (mixed widening measured no faster for the 32-bit formats: fp32 fused k = 100 384 against 333 us)
     __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
     {
         d[0] = f32_bits_to_raw(r.x);
@@ -115,6 +145,7 @@ template <> struct Fmt<CBGMRES_FP16> {
     static constexpr int VEC = 8, BYTES = 2;
     static constexpr bool SCALED = false;
     static constexpr double PRE = kPreF16;
+    static constexpr double PRE_EVEN = kPreF16Even;
     __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
     {
         half2_to_raw(r.x, d[0], d[1]);
@@ -132,6 +163,7 @@ template <> struct Fmt<CBGMRES_INT32> {
     static constexpr int VEC = 4, BYTES = 4;
     static constexpr bool SCALED = true;
     static constexpr double PRE = 1.0;
+    static constexpr double PRE_EVEN = 1.0;
     __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
     {
         d[0] = i32_to_double((int)r.x);
@@ -149,6 +181,7 @@ template <> struct Fmt<CBGMRES_INT16> {
     static constexpr int VEC = 8, BYTES = 2;
     static constexpr bool SCALED = true;
     static constexpr double PRE = 1.0;
+    static constexpr double PRE_EVEN = 1.0;
     __device__ static __forceinline__ void decode(const uint4 &r, double (&d)[VEC])
     {
         i16x2_to_doubles(r.x, d[0], d[1]);

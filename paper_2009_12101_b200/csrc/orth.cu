@@ -302,7 +302,7 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
 {
     using T = Tile<FMT, F>;
     constexpr int VEC = T::VEC, GV = T::GV, R = T::R;
-    constexpr double PRE = T::Fm::PRE;
+    constexpr double PRE = T::Fm::PRE, PRE_EVEN = T::Fm::PRE_EVEN;
     constexpr bool HAS_UPD = KIND != PASS_DOT, HAS_DOT = KIND != PASS_UPD;
     const int wi0 = c.half * T::WORDS_HALF + c.lane; // this lane's first 16-byte word in a column segment
     double *wt = c.wbuf + wslot * R;
@@ -330,7 +330,7 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
 #pragma unroll
             for (int v = 0; v < VEC; v += 2) {
                 const double2 t = *reinterpret_cast<const double2 *>(src + wswz<VEC>(src_s, (wi0 + f * 32) * VEC + v));
-                wreg[f * VEC + v] = (PRE == 1.0) ? t.x : t.x * PRE;
+                wreg[f * VEC + v] = (PRE_EVEN == 1.0) ? t.x : t.x * PRE_EVEN; // even rows: the entries widened by the conversion pipe
                 wreg[f * VEC + v + 1] = (PRE == 1.0) ? t.y : t.y * PRE;
             }
     };
@@ -452,14 +452,17 @@ __device__ __forceinline__ void consume_tile(const ConsumerCtx &c, const OrthArg
 #pragma unroll
     for (int i = 0; i < GV; ++i) p[i] = 0.0;
     for (int st = 0; st < c.nst; ++st) {
-        double coef[T::CPS]; // zero beyond k
+        double coef[T::CPS], coefE[T::CPS]; // zero beyond k; coefE: for the even entries (mixed widening)
 #pragma unroll
-        for (int i = 0; i < T::CPS; ++i) coef[i] = c.hs_s[st * T::STAGE_COLS + i * kChunkCols + c.cw];
+        for (int i = 0; i < T::CPS; ++i) {
+            coef[i] = c.hs_s[st * T::STAGE_COLS + i * kChunkCols + c.cw];
+            coefE[i] = (PRE_EVEN == PRE) ? coef[i] : coef[i] * (PRE_EVEN / PRE);
+        }
         mbar_wait(&c.full[ring.s], ring.ph);
         const unsigned char *stg = c.stages + (size_t)ring.s * T::STAGE;
         for_valid_chunks<FMT, F, RAGGED>(valid_chunks(st), stg, c.cw, wi0, rows, [&](int i, int f, const double(&d)[VEC]) {
 #pragma unroll
-            for (int v = 0; v < VEC; ++v) p[f * VEC + v] = fma(d[v], coef[i], p[f * VEC + v]);
+            for (int v = 0; v < VEC; ++v) p[f * VEC + v] = fma(d[v], (v & 1) ? coef[i] : coefE[i], p[f * VEC + v]);
         });
         if (KIND == PASS_UPD) {
             unsigned dep = 0; // p[f * VEC] has consumed word f of every column of the stage
@@ -903,7 +906,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
     using Fm = typename T::Fm;
     constexpr int VEC = T::VEC, B = T::B, R = T::R, NV = T::NV, RW = T::RW;
     constexpr int NOUT = NV >= 8 ? NV / 8 : 1; // finished rows per lane after the butterfly
-    constexpr double PRE = Fm::PRE;
+    constexpr double PRE = Fm::PRE, PRE_EVEN = Fm::PRE_EVEN;
     Ctl *ctl = a.ctl;
     const int ns = a.nstages;
 
@@ -1053,10 +1056,11 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
                 auto chunks = [&](auto nc_tag) {
                     constexpr int NC = decltype(nc_tag)::value;
                     uint4 raw[NC][WPL];
-                    double coef[NC];
+                    double coef[NC], coefE[NC]; // coefE: for the even entries (mixed widening)
 #pragma unroll
                     for (int c = 0; c < NC; ++c) {
                         coef[c] = hs_s[st * T::STAGE_COLS + c * kFGroups + j]; // zero beyond k
+                        coefE[c] = (PRE_EVEN == PRE) ? coef[c] : coef[c] * (PRE_EVEN / PRE);
 #pragma unroll
                         for (int q = 0; q < WPL; ++q)
                             raw[c][q] = (live[q] > 0) ? *reinterpret_cast<const uint4 *>(stg + c * T::BOX_BYTES + woff[q])
@@ -1071,7 +1075,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
 #pragma unroll
                             for (int v = 0; v < VEC; ++v) {
                                 if (ragged && v >= live[q]) d[v] = 0.0; // padding beyond n may decode to anything
-                                p[q * VEC + v] = fma(d[v], coef[c], p[q * VEC + v]);
+                                p[q * VEC + v] = fma(d[v], (v & 1) ? coef[c] : coefE[c], p[q * VEC + v]);
                             }
                         }
                 };
@@ -1115,7 +1119,7 @@ __global__ void __launch_bounds__(kOrthThreads, 1)
 #pragma unroll
                 for (int v = 0; v < VEC; v += 2) {
                     const double2 t2 = *reinterpret_cast<const double2 *>(w1w + rloc[q] + v);
-                    wreg[q * VEC + v] = (PRE == 1.0) ? t2.x : t2.x * PRE;
+                    wreg[q * VEC + v] = (PRE_EVEN == 1.0) ? t2.x : t2.x * PRE_EVEN;
                     wreg[q * VEC + v + 1] = (PRE == 1.0) ? t2.y : t2.y * PRE;
                 }
             __syncwarp(); // w1w is rewritten by the next tile only after every lane has read it

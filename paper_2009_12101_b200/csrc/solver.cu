@@ -230,8 +230,11 @@ int choose_spmv_kernel(cbgmres_ctx *h, int64_t n, int64_t nnz, int max_len)
     if (max_len > 64 && (double)max_len > 8.0 * mean) return 64;
     // regular: row-major from shared memory; blocks of 256 RPT / LPR rows must hold <= 3584 nonzeros
     const int len = (int)std::fmin((double)max_len, std::ceil(2.0 * mean));
-    if (len <= 3) return 132;  // 4 rows per thread
-    if (len <= 7) return 130;  // 2 rows per thread
+    // several rows per thread only while every one of the 2 x 148 persistent CTAs still gets at least twelve row blocks:
+    // with fewer, the pipeline ramp and the one-block imbalance show (C2, n = 1e6, 2 rows per thread: 6.6 blocks per CTA)
+    auto enough_blocks = [&](int rows_per_thread) { return n / (256 * rows_per_thread) >= 12 * 2 * kNumSMs; };
+    if (len <= 3 && enough_blocks(4)) return 132;  // 4 rows per thread
+    if (len <= 7 && enough_blocks(2)) return 130;  // 2 rows per thread
     if (len <= 14) return 129; // 1 row per thread
     if (len <= 28) return 146; // 2 lanes per row
     if (len <= 56) return 148; // 4 lanes per row
