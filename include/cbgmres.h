@@ -98,7 +98,8 @@ typedef struct {
     int32_t reorth_count; /* steps on which the second Gram-Schmidt pass ran */
     int32_t breakdown;    /* 1 if the last cycle ended through Fig. 1 line 12 */
     int32_t converged;    /* 1 iff the explicit residual met tau*||b|| */
-    int32_t spmv_kernel;  /* which SpMV variant ran (see cbgmres_set_option "spmv_kernel") */
+    int32_t spmv_kernel;  /* which SpMV variant ran (see cbgmres_set_option "spmv_kernel"); 1016 = the whole solve ran as
+                           * one kernel of a 16-CTA thread-block cluster (small systems, option "small_path") */
     double rel_res_recurrence; /* |g_{k+1}| / ||b|| at the end of the last cycle */
     double rel_res_true;       /* last explicit ||b - A x|| / ||b|| */
     double b_norm;
@@ -150,7 +151,10 @@ const char *cbgmres_last_error(cbgmres_handle_t h);
  * "profile": N > 0 = time the kernels of every N-th Arnoldi step of a cycle with CUDA events (see
  * cbgmres_profile_get; 1 = every step), default 0.  "pdl": 1 (default) = launch the step kernels with
  * programmatic stream serialisation (each parks in griddepcontrol.wait until its predecessor is done).
- * "orth_fuse": 1 (default) = fuse the first update with the second pass's multi-dot (one read of V).
+ * "small_path": 1 (default) = a system whose compressed basis, matrix and vectors fit the distributed shared memory of
+ * one 16-CTA thread-block cluster (about 3 MB: e.g. n = 4,096, m = 50 in fp64) is solved by ONE kernel launch with
+ * cluster barriers in place of kernel boundaries (preconditioner none or scalar Jacobi, restart <= 128); 0 = always the
+ * large path.  "orth_fuse": 1 (default) = fuse the first update with the second pass's multi-dot (one read of V).
  * "orth_fused_rows": the fused pass maps warps to rows and adds the update's partial sums with shuffles
  * (orth_fused_kernel) for 2 (default) = the 16-bit formats, 1 = every reduced format, 0 = never (the column-mapped
  * kind of orth_kernel with its shared-memory reduction).

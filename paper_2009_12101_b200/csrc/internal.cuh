@@ -105,6 +105,7 @@ struct CsrView {
     int nblk;
     int reduce_lanes;       // lanes sharing a row in the streaming kernel's row reduction (power of two)
     int kernel;             // 2,4,8,16,32 lanes per row, or 64 = streaming
+    int slab_nnz;           // nonzeros of the fullest of 16 equal row slabs (small-system path; 0 = not applicable)
 };
 
 // ---- launchers (each enqueues on `s` and returns the number of kernels launched) -------------
@@ -135,6 +136,12 @@ int launch_diag_scale(cudaStream_t s, int64_t n, double *x, const double *d, int
 int launch_bj4_setup(cudaStream_t s, const CsrView &A, double *inv);
 int launch_bj4_axpy(cudaStream_t s, int64_t n, const double *inv, const double *t, double *x); // x += M^-1 t (Fig. 1 l.17)
 int launch_fill_zero(cudaStream_t s, int64_t n, double *x);
+
+// Small systems: the whole solve in one kernel of a 16-CTA cluster (cluster.cu)
+int small_slab_nnz(cudaStream_t s, int64_t n, const int32_t *d_row_ptr, int *d_scratch);
+bool small_fits(int64_t n, int slab_nnz, int m, int format);
+int launch_small_solve(cudaStream_t s, const Scratch &sc, const CsrView &A, const double *b, double *x, const CycleState &cyc,
+                       int m, int format, int slab_nnz);
 
 int launch_row_stats(cudaStream_t s, int64_t n, const int32_t *d_row_ptr, int *d_out);
 

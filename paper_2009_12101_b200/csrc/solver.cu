@@ -45,6 +45,7 @@ struct cbgmres_ctx {
     int opt_poll = 1;
     int opt_seg_kb = 0; // column-segment size of the Gram-Schmidt passes (0 = auto)
     int opt_fuse = 1;   // fused update + second-pass multi-dot
+    int opt_small = 1;  // small systems: the whole solve in one kernel of a 16-CTA cluster (cluster.cu)
     int64_t launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     // optional per-kernel timing ("profile" option): event pairs around the launches of one cycle
@@ -230,11 +231,10 @@ int choose_spmv_kernel(cbgmres_ctx *h, int64_t n, int64_t nnz, int max_len)
     if (max_len > 64 && (double)max_len > 8.0 * mean) return 64;
     // regular: row-major from shared memory; blocks of 256 RPT / LPR rows must hold <= 3584 nonzeros
     const int len = (int)std::fmin((double)max_len, std::ceil(2.0 * mean));
-    // several rows per thread only while every one of the 2 x 148 persistent CTAs still gets at least twelve row blocks:
-    // with fewer, the pipeline ramp and the one-block imbalance show (C2, n = 1e6, 2 rows per thread: 6.6 blocks per CTA)
-    auto enough_blocks = [&](int rows_per_thread) { return n / (256 * rows_per_thread) >= 12 * 2 * kNumSMs; };
-    if (len <= 3 && enough_blocks(4)) return 132;  // 4 rows per thread
-    if (len <= 7 && enough_blocks(2)) return 130;  // 2 rows per thread
+    // (halving the row blocks when a CTA gets fewer than twelve -- C2, n = 1e6: 6.6 blocks per CTA -- measured no gain:
+    // 31.4 against 29.7 us, L2 flushed)
+    if (len <= 3) return 132;  // 4 rows per thread
+    if (len <= 7) return 130;  // 2 rows per thread
     if (len <= 14) return 129; // 1 row per thread
     if (len <= 28) return 146; // 2 lanes per row
     if (len <= 56) return 148; // 4 lanes per row
@@ -271,6 +271,9 @@ int register_matrix(cbgmres_ctx *h, int64_t n, int64_t nnz, const int32_t *rp, c
         const double mean = (double)nnz / (double)n; // about 4 products per lane
         h->A.reduce_lanes = mean <= 6.0 ? 1 : mean <= 12.0 ? 2 : mean <= 24.0 ? 4 : mean <= 48.0 ? 8 : mean <= 96.0 ? 16 : 32;
     }
+    // small systems: how many nonzeros the fullest of 16 equal row slabs holds (decides whether the cluster path fits)
+    h->A.slab_nnz = small_slab_nnz(h->stream, n, rp, h->d_stats + 16);
+    if (h->A.slab_nnz) h->launches += 1;
     h->has_matrix = true;
     return CBGMRES_OK;
 }
@@ -374,6 +377,10 @@ int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value)
     }
     if (!strcmp(name, "orth_fuse")) {
         h->opt_fuse = value != 0;
+        return CBGMRES_OK;
+    }
+    if (!strcmp(name, "small_path")) {
+        h->opt_small = value != 0;
         return CBGMRES_OK;
     }
     if (!strcmp(name, "orth_fused_rows")) {
@@ -610,7 +617,26 @@ int cbgmres_solve(cbgmres_handle_t h, const double *d_b, double *d_x, const cbgm
     }
     return CBGMRES_OK;
     };
-    rc = cycles();
+    // Small systems (basis + matrix + vectors within the distributed shared memory of one 16-CTA cluster): the whole
+    // solve is ONE kernel (cluster.cu).  -1 = not applicable / launch refused: the large path runs.
+    auto small = [&]() -> int {
+        if (!h->opt_small || bj4 || !small_fits(n, h->A.slab_nnz, m, fmt)) return -1;
+        const int nl = launch_small_solve(s, h->sc, A, d_b, d_x, cy, m, fmt, h->A.slab_nnz);
+        if (!nl) { // e.g. no room for a 16-CTA cluster on this device right now: not an error, use the large path
+            h->lc.launch_error = cudaSuccess;
+            h->lc.launch_kernel = "";
+            (void)cudaGetLastError();
+            return -1;
+        }
+        h->launches += nl;
+        CK(cudaMemcpyAsync(h->h_ctl, dctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
+        CK(cudaStreamSynchronize(s));
+        CK(cudaGetLastError());
+        out->spmv_kernel = 1016;
+        return CBGMRES_OK;
+    };
+    rc = small();
+    if (rc == -1) rc = cycles();
     if (jacobi) { // l.17: x = M^-1 u -- on every exit, also the failed ones (x then holds the last iterate reached)
         h->launches += launch_diag_scale(s, n, d_x, pdiag, 1);
         if (rc != CBGMRES_OK) cudaStreamSynchronize(s);

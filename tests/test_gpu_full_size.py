@@ -223,9 +223,11 @@ def test_full_size_solve_matches_cached_oracle(full_solvers, case, fmt):
     if rule == "strict":
         assert abs(r.restarts - o["restarts"]) <= 1
         assert abs(r.reorth_count - o["reorth_count"]) <= max(2, 0.02 * o["reorth_count"])
-    # the first 40 steps are before any decorrelation: the recurrence residuals agree to the format's roundoff
-    k = min(40, r.iters, o["iters"])
+    # the first steps are before any decorrelation: the recurrence residuals agree to the format's roundoff (40 steps on
+    # the stencils; 12 on the power-law matrix, whose quantised histories part within some tens of steps: reading Q11)
+    c4 = case.startswith("C4")
+    k = min(12 if c4 else 40, r.iters, o["iters"])
     hg, ho = np.asarray(r.rec_history[:k]), np.asarray(o["rec_history"][:k])
-    assert np.all(np.abs(hg - ho) <= HIST_TOL[fmt] * ho * (100 if case.startswith("C4") else 1))
+    assert np.all(np.abs(hg - ho) <= HIST_TOL[fmt] * ho * (100 if c4 else 1))
     print(f"[full-size] {case} {fmt}: gpu iters {r.iters} restarts {r.restarts} | oracle {o['iters']} {o['restarts']} "
           f"draws {sorted(draws)} | rule {rule} | true residual gpu {true:.3e} oracle {o['rel_res_true_recomputed']:.3e}")

@@ -490,3 +490,72 @@ def test_two_handles_with_different_options_do_not_interfere():
     finally:
         for s in hs:
             s.destroy()
+
+
+# ---- small systems: the whole solve as one kernel of a 16-CTA cluster (csrc/cluster.cu) ---------------------------
+
+def _solve_opt(p, fmt, small, restart=None, rel_tol=None, max_iters=None, precond="none", reorth="cond", x0=None):
+    from paper_2009_12101_b200 import Solver
+
+    s = Solver(0)
+    try:
+        s.set_option("small_path", small)
+        s.set_matrix(p.A.row_ptr, p.A.col_idx, p.A.vals)
+        x, r = s.solve(p.b, p.x0 if x0 is None else x0, restart or p.restart, rel_tol or p.rel_tol, max_iters or p.max_iters,
+                       fmt, history=True, precond=precond, reorth=reorth)
+        return x.cpu().numpy(), r
+    finally:
+        s.destroy()
+
+
+@pytest.mark.parametrize("fmt", oracle.FORMATS)
+@pytest.mark.parametrize("cfg,kw,m,precond", [("C1", {}, 50, "none"), ("C1", {"grid": 16}, 10, "none"), ("C2", {"grid": 12}, 30, "none"),
+                                             ("C4", {"n": 3000}, 50, "jacobi"), ("C5", {"grid": 9}, 128, "none")])
+def test_small_system_cluster_path(cfg, kw, m, precond, fmt):
+    """The cluster kernel against the oracle (iteration counts, residuals) and against the large path of the same
+    library (same algorithm, different summation order: fp64 histories agree to rounding)."""
+    from workloads import Problem
+
+    q = make_config(cfg, **kw)
+    p = Problem(f"{cfg}-small", q.A, q.b, q.x0, m, q.rel_tol, 3000, oracle.FORMATS, {})
+    xs, rs = _solve_opt(p, fmt, 1, precond=precond)
+    xl, rl = _solve_opt(p, fmt, 0, precond=precond)
+    assert rs.spmv_kernel == 1016 and rl.spmv_kernel != 1016  # the two paths really ran
+    run = lambda: oracle.gmres(p.A, p.b, p.x0, m, p.rel_tol, 3000, fmt, precond=precond)
+    ref = run()
+    assert rs.converged == ref.converged == rl.converged
+    check_iters(rs.iters, ref.iters, fmt, f"{cfg}-small", run=run)
+    ts, tr = _true_rel_res(p, xs), _true_rel_res(p, ref.x)
+    assert ts <= p.rel_tol * (1 + 1e-9) and ts <= 10 * tr and tr <= 10 * ts
+    assert rs.rel_res_true == pytest.approx(ts, rel=1e-6)
+    assert rs.b_norm == pytest.approx(ref.b_norm, rel=1e-13)
+    if fmt == "fp64":
+        assert rs.iters == rl.iters == ref.iters and rs.restarts == ref.restarts and rs.reorth_count == ref.reorth_count
+        live = ref.rec_history > 1e-7
+        assert np.allclose(rs.rec_history[live], ref.rec_history[live], rtol=1e-7)
+        assert np.allclose(rs.rec_history[live], rl.rec_history[live], rtol=1e-7)
+
+
+def test_small_system_cluster_path_edge_cases():
+    """Exact x0, iteration bound inside a cycle, restart length 1, a tiny dense system with x0 != 0, l.12."""
+    p = make_config("C1", grid=16)
+    xs_ = p.meta["xstar"]
+    x, r = _solve_opt(p, "fp64", 1, restart=10, rel_tol=1e-10, max_iters=50, x0=xs_)
+    assert r.converged and r.iters == 0 and r.restarts == 0 and np.array_equal(x, xs_) and r.spmv_kernel == 1016
+    x, r = _solve_opt(p, "fp64", 1, restart=10, rel_tol=1e-14, max_iters=25)
+    ref = oracle.gmres(p.A, p.b, p.x0, 10, 1e-14, 25, "fp64")
+    assert (not r.converged) and r.status == 16 and r.iters == 25 and r.restarts == 3
+    assert _true_rel_res(p, x) == pytest.approx(ref.rel_res_true, rel=1e-6)
+    assert np.allclose(r.rec_history, ref.rec_history, rtol=1e-8)
+    x, r = _solve_opt(p, "int16", 1, restart=1, rel_tol=1e-3, max_iters=500)
+    ref = oracle.gmres(p.A, p.b, p.x0, 1, 1e-3, 500, "int16")
+    assert r.converged == ref.converged and abs(r.iters - ref.iters) <= max(2, 0.02 * ref.iters)
+    for n, seed in ((1, 40), (3, 41), (33, 42), (64, 43)):
+        A, Ad, b = random_dense_system(n, seed)
+        from workloads import Problem
+
+        x0 = np.random.default_rng(seed).standard_normal(n)
+        q = Problem("tiny", A, b, x0, n, 1e-13, 4 * n + 4, ("fp64",), {})
+        x, r = _solve_opt(q, "fp64", 1)
+        assert r.spmv_kernel == 1016 and r.converged and r.iters <= n + 1
+        assert np.linalg.norm(x - np.linalg.solve(Ad, b)) <= 1e-10 * np.linalg.norm(x)
