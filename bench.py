@@ -188,7 +188,7 @@ def run_reference(args) -> int:
 
 
 # ---- our arm ----------------------------------------------------------------------------------------
-def _solve_all_formats(solver, p, dev, host=None, profile=False, precond=None, max_iters=None):
+def _solve_all_formats(solver, p, dev, host=None, profile=False, precond=None, max_iters=None, reorth="cond"):
     """One step: one solve per storage format.  Returns {fmt: SolveResult}."""
     out = {}
     pc = PRECOND if precond is None else precond
@@ -196,7 +196,7 @@ def _solve_all_formats(solver, p, dev, host=None, profile=False, precond=None, m
         if host is None:
             if profile:
                 solver.profile_reset()
-            _, r = solver.solve(dev["b"], dev["x0"], p.restart, p.rel_tol, max_iters or p.max_iters, fmt, precond=pc)
+            _, r = solver.solve(dev["b"], dev["x0"], p.restart, p.rel_tol, max_iters or p.max_iters, fmt, precond=pc, reorth=reorth)
             if profile:
                 r.prof = solver.profile_get()
         else:
@@ -426,6 +426,11 @@ def run_ours(args) -> int:
         extras["msweep"] = {"workload": args.workload, "cycles": 3, "protocol": "full cycles of m steps, tolerance 0 (numerical effects ignored, PAPER.md:294)",
                             "rows": [{k: (round(v, 4) if isinstance(v, float) else v) for k, v in r.items()} for r in rows]}
         _log("msweep done")
+        # -- the two-read regime of the paper's memop model (PAPER.md:116 assumes l.7 never fires): same workload, reorth = never --
+        never = [_solve_all_formats(solver, p, dev, reorth="never") for _ in range(2)][1:]
+        extras_never = {"n": n, "nnz": nnz, "restart": p.restart, "rel_tol": p.rel_tol, "precond": PRECOND, "reorth": "never",
+                        "formats": _format_table(p, never, peak)}
+        _log("reorth=never done")
         # -- C3 (BASELINE.json configs[2]): S2 / S3 / S3+S2' / S4 timed separately at n = 4,194,304 --
         rows = microbench.run(solver, C3_N, list(C3_KS), list(FORMATS), reps=10, flush=True)
         extras["c3"] = {"n": C3_N, "ks": list(C3_KS), "l2": "512 MB written between launches (nothing L2-resident)",
@@ -436,7 +441,8 @@ def run_ours(args) -> int:
         solver.destroy()
         solver = None
         per_config = {args.workload + ("" if PRECOND == "none" else "+" + PRECOND): {
-            "n": n, "nnz": nnz, "restart": p.restart, "rel_tol": p.rel_tol, "precond": PRECOND, "formats": per_format}}
+            "n": n, "nnz": nnz, "restart": p.restart, "rel_tol": p.rel_tol, "precond": PRECOND, "reorth": "cond", "formats": per_format},
+            args.workload + " reorth=never": extras_never}
         for name, pc, bound in (("C1", "none", None), ("C2", "none", None), ("C4", "none", 500), ("C4", "jacobi", 1000),
                                 ("C4", "block_jacobi4", 1000)):
             if name == args.workload and pc == PRECOND:

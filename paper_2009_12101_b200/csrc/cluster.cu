@@ -30,7 +30,7 @@ namespace cg = cooperative_groups;
 namespace cbg {
 
 constexpr int kClusterCtas = 16;   // non-portable cluster size (opt-in), all of one GPC's worth of SMs
-constexpr int kSmallThreads = 512;
+constexpr int kSmallThreads = 256; // 8 warps x up to 255 registers: the many shared-memory pointers of the kernel stay in registers
 constexpr int kSmallMaxRestart = 128;
 constexpr int kSmallSmemBytes = 200 * 1024;
 
@@ -146,8 +146,8 @@ template <int FMT> __global__ void __launch_bounds__(kSmallThreads, 1) small_sol
     auto exchange = [&](int count, int max_slot) {
         __syncthreads(); // loc[] complete
         double *mine = part + ((size_t)pbuf * C + rank) * pstride;
-        { // warp q sends this CTA's partial sums to CTA q (16 warps, 16 destinations: all in flight together)
-            double *remote = cluster.map_shared_rank(mine, warp);
+        for (int dst = warp; dst < C; dst += NW) { // warp q sends this CTA's partial sums to CTAs q, q + 8: all in flight together
+            double *remote = cluster.map_shared_rank(mine, dst);
             for (int i = lane; i < count; i += 32) remote[i] = loc[i];
         }
         cluster.sync();
@@ -185,11 +185,13 @@ template <int FMT> __global__ void __launch_bounds__(kSmallThreads, 1) small_sol
     };
     // own rows of a vector into every CTA's copy of the full vector (the caller separates it from readers by a barrier)
     auto allgather = [&](const double *own) {
-        double *remote = cluster.map_shared_rank(vfull, warp) + (size_t)rank * nr; // warp q -> CTA q
-        if ((nr & 1) == 0) {
-            for (int r = 2 * lane; r < nr; r += 64) *reinterpret_cast<double2 *>(remote + r) = *reinterpret_cast<const double2 *>(own + r);
-        } else {
-            for (int r = lane; r < nr; r += 32) remote[r] = own[r];
+        for (int dst = warp; dst < C; dst += NW) { // warp q -> CTAs q, q + 8
+            double *remote = cluster.map_shared_rank(vfull, dst) + (size_t)rank * nr;
+            if ((nr & 1) == 0) {
+                for (int r = 2 * lane; r < nr; r += 64) *reinterpret_cast<double2 *>(remote + r) = *reinterpret_cast<const double2 *>(own + r);
+            } else {
+                for (int r = lane; r < nr; r += 32) remote[r] = own[r];
+            }
         }
     };
     auto spmv_rows = [&](bool residual, double &ss, double &am) { // w = A vfull (or b - A vfull) on the own rows

@@ -381,6 +381,21 @@ inline cudaError_t launch_chain(const Scratch &sc, const char *name, void (*kern
 // CTA-scope MEMBAR.SC also closes the window but costs ~400 cycles per release).  `dep` must be
 // computed from results that consumed every load from the slot; the warp vote needs it from all 32
 // lanes and its result is an input of the arrive, so neither can be scheduled before the uses.
+// Why this is sufficient (there is no racecheck on this pool, so the argument is written down):
+//  (1) Hardware: an LDS whose result has been consumed by an arithmetic instruction has completed -- the
+//      scoreboard releases the consumer only when the loaded value is in the register file -- so once `dep` exists,
+//      no read of the slot by this lane is still in flight.
+//  (2) Compiler: `dep` is data-dependent on every value loaded from the slot (the callers fold one accumulator per
+//      128-bit load into it); the ballot's predicate depends on `dep`, the ballot needs all 32 lanes, and its result `b`
+//      is an INPUT operand of the asm volatile arrive ("memory" clobber): the arrive cannot be hoisted above the
+//      ballot, nor the ballot above the last use, in any lane.  (The comparison constant is a NaN pattern no
+//      accumulator produces; the branch is never taken -- it only keeps the dependency alive.)
+//  (3) Memory model: mbarrier.arrive has release semantics at CTA scope, the producer's try_wait acquires; the
+//      producer's next cp.async.bulk into the slot is issued after that wait, so it is ordered after the reads of (1).
+//      The reads are generic-proxy reads, the refill an async-proxy write: a write-after-read across the proxies needs
+//      no proxy fence (only generic-proxy WRITES to the slot do, which is why the ragged w tile, patched by hand, issues
+//      fence.proxy.async before its arrive).
+// Regression tests: test_multidot_many_tiles_per_cta_repeats_bitwise, test_full_size_c2_solve_is_bitwise_repeatable.
 __device__ __forceinline__ unsigned dep_bits(double x) { return (unsigned)__double2hiint(x); }
 __device__ __forceinline__ void mbar_arrive_after_use(uint64_t *bar, int lane, unsigned dep)
 {
