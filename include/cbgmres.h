@@ -146,7 +146,9 @@ int cbgmres_destroy(cbgmres_handle_t h);
 const char *cbgmres_last_error(cbgmres_handle_t h);
 
 /* Tuning / test knobs, by name.  "spmv_kernel": 0 = choose from the row-length statistics,
- * L in {2,4,8,16,32} = L lanes per row, 64 = nnz-balanced streaming kernel.  "poll": 1 (default)
+ * L in {2,4,8,16,32} = L lanes per row, 64 = nnz-balanced streaming kernel, 65 = the same with the matrix stream staged
+ * in shared memory by bulk copies, 129/130/132 = row-major kernel with 1/2/4 rows per thread, 146/148/152 = with 2/4/8
+ * lanes per row.  "poll": 1 (default)
  * = the host stops launching a cycle's remaining steps once the device reports it left the cycle.
  * "profile": N > 0 = time the kernels of every N-th Arnoldi step of a cycle with CUDA events (see
  * cbgmres_profile_get; 1 = every step), default 0.  "pdl": 1 (default) = launch the step kernels with

@@ -147,6 +147,6 @@ int launch_row_stats(cudaStream_t s, int64_t n, const int32_t *d_row_ptr, int *d
 
 // row-partition metadata for the streaming SpMV (set_matrix)
 cudaError_t build_row_blocks(cudaStream_t s, int64_t n, int64_t nnz, const int32_t *d_row_ptr, int4 **d_desc_out,
-                             int *nblk_out);
+                             int *nblk_out, int kernel);
 
 } // namespace cbg

@@ -262,9 +262,9 @@ int register_matrix(cbgmres_ctx *h, int64_t n, int64_t nnz, const int32_t *rp, c
     CK(cudaMemcpyAsync(&max_len, h->d_stats, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
     h->A.kernel = choose_spmv_kernel(h, n, nnz, max_len);
-    if (h->A.kernel == 64) {
+    if (h->A.kernel == 64 || h->A.kernel == 65) {
         int nblk = 0;
-        CK(build_row_blocks(h->stream, n, nnz, rp, &h->owned_blk_row, &nblk));
+        CK(build_row_blocks(h->stream, n, nnz, rp, &h->owned_blk_row, &nblk, h->A.kernel));
         h->launches += 1;
         h->A.blk_desc = h->owned_blk_row;
         h->A.nblk = nblk;
@@ -354,9 +354,9 @@ int cbgmres_set_option(cbgmres_handle_t h, const char *name, int64_t value)
 {
     if (!h || !name) return CBGMRES_E_INVALID;
     if (!strcmp(name, "spmv_kernel")) {
-        if (value != 0 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32 && value != 64 &&
+        if (value != 0 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32 && value != 64 && value != 65 &&
             value != 129 && value != 130 && value != 132 && value != 146 && value != 148 && value != 152)
-            return fail(h, CBGMRES_E_INVALID, "spmv_kernel must be 0, 2, 4, 8, 16, 32, 64, 129, 130, 132, 146, 148 or 152");
+            return fail(h, CBGMRES_E_INVALID, "spmv_kernel must be 0, 2, 4, 8, 16, 32, 64, 65, 129, 130, 132, 146, 148 or 152");
         h->opt_spmv_kernel = (int)value;
         return CBGMRES_OK;
     }

@@ -352,7 +352,7 @@ def test_cgs_closed_form(solver, fmt):
 
 # ------------------------------------------------------------------------------------------ SpMV
 @pytest.mark.parametrize("name,kw", [("C1", {}), ("C2", {"grid": 30}), ("C4", {"n": 60000}), ("C5", {"grid": 20})])
-@pytest.mark.parametrize("kernel", [0, 2, 4, 8, 16, 32, 64, 129, 130, 132, 146, 148, 152])
+@pytest.mark.parametrize("kernel", [0, 2, 4, 8, 16, 32, 64, 65, 129, 130, 132, 146, 148, 152])
 def test_spmv_matches_oracle(name, kw, kernel):
     from paper_2009_12101_b200 import Solver
 
@@ -389,7 +389,7 @@ def test_spmv_empty_rows_and_long_rows():
     A = CSR(n, M.indptr.astype(np.int32), M.indices.astype(np.int32), M.data.astype(np.float64))
     x = rng.standard_normal(n)
     y_ref, rowabs = oracle.ref_spmv(A, x)
-    for kernel in (0, 8, 32, 64):
+    for kernel in (0, 8, 32, 64, 65):
         s = Solver(0)
         try:
             s.set_option("spmv_kernel", kernel)
