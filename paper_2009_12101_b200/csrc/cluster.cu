@@ -208,17 +208,24 @@ template <int FMT> __global__ void __launch_bounds__(kSmallThreads, 1) small_sol
     };
     // partial inner products of the stored vectors 0 .. j-1 with w over the own rows -> loc[0 .. j)
     auto dots = [&](int j) {
-        for (int c = warp; c < j; c += NW) {
-            const unsigned char *col = basis + (size_t)c * nr * B;
-            double s0 = 0.0, s1 = 0.0;
-            int r = lane;
-            for (; r + 32 < rows; r += 64) {
-                s0 = fma(Fm::decode_one(col, r), w[r], s0);
-                s1 = fma(Fm::decode_one(col, r + 32), w[r + 32], s1);
+        // a warp takes four columns at a time: four independent chains per lane and four shuffle reductions in flight
+        for (int c0 = 4 * warp; c0 < j; c0 += 4 * NW) {
+            double s4[4] = {0.0, 0.0, 0.0, 0.0};
+            const unsigned char *col[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) col[q] = basis + (size_t)min(c0 + q, j - 1) * nr * B;
+            for (int r = lane; r < rows; r += 32) {
+                const double wr = w[r];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) s4[q] = fma(Fm::decode_one(col[q], r), wr, s4[q]);
             }
-            if (r < rows) s0 = fma(Fm::decode_one(col, r), w[r], s0);
-            const double s = warp_sum(s0 + s1);
-            if (lane == 0) loc[c] = s;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) s4[q] = warp_sum(s4[q]);
+            if (lane == 0) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    if (c0 + q < j) loc[c0 + q] = s4[q];
+            }
         }
     };
     // w_r -= sum_c payload[r, c] * hs_c on the own rows; partial norms of the new w
