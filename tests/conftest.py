@@ -3,6 +3,10 @@ import sys
 
 import pytest
 
+# The oracle's OpenMP threads spin at their barriers by default; on a box whose cores are shared with anything else that
+# turns the many tiny solves of the CPU suite from seconds into tens of minutes.  Must be set before libgomp loads.
+os.environ.setdefault("OMP_WAIT_POLICY", "passive")
+
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
