@@ -41,6 +41,8 @@ def _short(name: str) -> str:
 
 def _family(kernel: str) -> str:
     k = _short(kernel)
+    if "orth_fused" in k:  # the row-mapped fused update + multi-dot (template arguments: format, words per lane)
+        return "update_multidot"
     if "orth" in k:
         kind = k.rstrip(">").split(",")[-1].strip()
         return {"0": "multidot", "1": "update", "2": "update_multidot"}.get(kind, k)
@@ -98,7 +100,11 @@ STALLS = ["long_scoreboard", "short_scoreboard", "barrier", "wait", "math_pipe_t
 
 
 def _raw_rows(rep):
-    txt = subprocess.run(["ncu", "-i", rep, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
+    if rep.endswith(".csv"):  # the raw page already exported on the GPU box (`ncu -i REP --page raw --csv > REP_raw.csv`)
+        with open(rep) as f:
+            txt = f.read()
+    else:
+        txt = subprocess.run(["ncu", "-i", rep, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
     rd = list(csv.reader(io.StringIO(txt)))
     hdr, units, data = rd[0], rd[1], rd[2:]
     idx = {h: i for i, h in enumerate(hdr)}
