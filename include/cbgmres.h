@@ -225,6 +225,30 @@ int cbgmres_k_store_bj4(cbgmres_handle_t h, int32_t format, int64_t n, const dou
  * *d_nrm2 <- ||w||_2 (omega, line 4) from the same pass. */
 int cbgmres_k_spmv(cbgmres_handle_t h, const double *d_v, double *d_w, double *d_nrm2);
 
+/* ---- an entry point that allocates nothing ----------------------------------------------------
+ * S2 (Fig. 1 line 5) as cbgmres_k_multidot computes it -- d_h[c] <- sum_i dec(V)[i,c] * d_w[i],
+ * the same kernels, the same bits -- for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * serving loops, harnesses that forbid allocation).  It takes no handle (cbgmres_create allocates): the scratch
+ * the reduction goes through (CTA partial sums, the last-block-done ticket) is a file-scope device array of
+ * CBGMRES_NOALLOC_SCRATCH_BYTES that every GPU loading the library holds until the process exits.
+ *   device   CUDA device ordinal the buffers live on (made current); stream: a cudaStream_t of that device
+ *            (borrowed; the call only enqueues: a memset of the control block, then one kernel).
+ *   format, n, ld, k, d_V, d_scales, d_w, d_h: as cbgmres_k_multidot; all DEVICE pointers, caller-owned.
+ *   k > CBGMRES_NOALLOC_MAX_K is rejected with CBGMRES_E_INVALID (nothing enqueued); k == 0 is a no-op.
+ * The call makes no cudaMalloc / cudaFree / allocating library call.  All calls on one GPU share the array,
+ * which keeps the last call's contents (what must start at zero is cleared on `stream` first): calls that
+ * overlap on the GPU -- two streams, two host threads -- race; serialise them.
+ * cbgmres_noalloc_setup(device) takes the array's device address (cudaGetSymbolAddress, once per device);
+ * the first k_multidot_noalloc call on a device does it itself, so calling it is only needed to keep that
+ * one-time step out of a region where it is unwelcome.  Errors: the status code, and a per-thread message
+ * from cbgmres_noalloc_last_error(). */
+#define CBGMRES_NOALLOC_MAX_K 128
+#define CBGMRES_NOALLOC_SCRATCH_BYTES 635392
+int cbgmres_noalloc_setup(int32_t device);
+int cbgmres_k_multidot_noalloc(int32_t device, void *stream, int32_t format, int64_t n, int64_t ld, int32_t k,
+                               const void *d_V, const double *d_scales, const double *d_w, double *d_h);
+const char *cbgmres_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -30,8 +30,10 @@ EXPORTS = (
     "cbgmres_workspace_bytes_host", "cbgmres_solve_host", "cbgmres_destroy", "cbgmres_last_error",
     "cbgmres_set_option", "cbgmres_launch_count", "cbgmres_k_compress", "cbgmres_k_decode", "cbgmres_k_multidot",
     "cbgmres_k_update", "cbgmres_k_update_multidot", "cbgmres_k_store", "cbgmres_k_spmv", "cbgmres_profile_get", "cbgmres_profile_reset",
-    "cbgmres_k_bj4_setup", "cbgmres_k_store_bj4",
+    "cbgmres_k_bj4_setup", "cbgmres_k_store_bj4", "cbgmres_noalloc_setup", "cbgmres_k_multidot_noalloc",
+    "cbgmres_noalloc_last_error",
 )
+NOALLOC_MAX_K = 128  # CBGMRES_NOALLOC_MAX_K
 PROF_FAMILIES = ("spmv", "multidot", "update", "store", "xupdate", "residual", "update_multidot")
 
 
@@ -90,8 +92,12 @@ def load_library(path: str = LIB_PATH):
     L.cbgmres_k_store_bj4.argtypes = [vp, i32, i64, vp, dbl, dbl, vp, vp, vp, vp]
     L.cbgmres_profile_get.argtypes = [vp, i32, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i64)]
     L.cbgmres_profile_reset.argtypes = [vp]
+    L.cbgmres_noalloc_setup.argtypes = [i32]
+    L.cbgmres_k_multidot_noalloc.argtypes = [i32, vp, i32, i64, i64, i32, vp, vp, vp, vp]
+    L.cbgmres_noalloc_last_error.argtypes = []
+    L.cbgmres_noalloc_last_error.restype = C.c_char_p
     for name in EXPORTS:
-        if name not in ("cbgmres_last_error", "cbgmres_launch_count"):
+        if name not in ("cbgmres_last_error", "cbgmres_launch_count", "cbgmres_noalloc_last_error"):
             getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -113,6 +119,23 @@ def payload_dtype(fmt: str):
 
 def _ptr(t):
     return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+def k_multidot_noalloc(fmt: str, V, scales, w, h, n: int | None = None, k: int | None = None):
+    """cbgmres_k_multidot_noalloc: h[:k] <- V[:k]^T w with the library's static device scratch -- no handle, no
+    allocation inside the call (the caller passes the output `h`, a device tensor of >= k doubles).  Enqueues on
+    torch's current stream of V's device.  k > NOALLOC_MAX_K raises CbgmresError (E_INVALID)."""
+    torch = _torch()
+    L = load_library()
+    k = V.shape[0] if k is None else k
+    n = w.numel() if n is None else n
+    dev = V.device.index if V.device.index is not None else torch.cuda.current_device()
+    stream = torch.cuda.current_stream(dev).cuda_stream
+    rc = L.cbgmres_k_multidot_noalloc(dev, C.c_void_p(stream), FORMAT_CODE[fmt], n, V.shape[1], k, _ptr(V), _ptr(scales),
+                                      _ptr(w), _ptr(h))
+    if rc != 0:
+        raise CbgmresError(rc, (L.cbgmres_noalloc_last_error() or b"").decode())
+    return h[:k]
 
 
 @dataclass

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcbgmres.so")
-SOURCES = ["orth.cu", "store.cu", "spmv.cu", "small.cu", "cluster.cu", "solver.cu"]
+SOURCES = ["orth.cu", "store.cu", "spmv.cu", "small.cu", "cluster.cu", "solver.cu", "noalloc.cu"]
 HEADERS = ["internal.cuh", "device_utils.cuh", os.path.join("..", "..", "include", "cbgmres.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
