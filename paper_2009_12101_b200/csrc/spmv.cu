@@ -201,8 +201,27 @@ template <int LANES, int U> __global__ void __launch_bounds__(256) spmv_vec_kern
 // from there (g lanes per row, a warp per very long row), in a fixed order.  The matrix is read once
 // per Arnoldi step and the basis passes stream hundreds of MB in between, so its lines are marked
 // evict-first in L2: the 126 MB L2 is kept for the basis and the vectors.
+// What bounds it on a power-law matrix is how many scattered 8-byte gathers of x an SM has in flight and for how much
+// of the time (ncu on C4, n = 2e6, nnz = 4.2e7, before round 2: issue slots 15 % busy, 0.25 eligible warps per scheduler,
+// no unit above 30 % of its peak; 587 us against 217 us for a bare torch.index_select of the same entries).  Round 2:
+//  (1) the gathers are volatile asm like the index / value loads.  Written as plain loads the compiler interleaved
+//      gather -> multiply -> store per item to save registers (40 registers, two or three gathers in flight per thread:
+//      the "all loads first" of the source was not what ran): 587 -> 385 us;
+//  (2) the values go global -> shared memory with cp.async, so no register holds them while the gathers are in flight
+//      (64 registers: four CTAs per SM with twelve gathers per thread), and the row pointers of a pass of phase 2 are
+//      fetched under the previous pass (volatile loads again): 385 -> 333 us (372 us with L2 flushed; 359 us inside
+//      a Jacobi-preconditioned C4 solve, 630 us before).
+// Tried on top and dropped: the next block's descriptor and column indices prefetched into shared memory with cp.async
+// while this block's gathers are in flight (18 KB more shared memory and a spill at four CTAs per SM: 478 us; 351 us at
+// three CTAs per SM); eight items at five or six CTAs per SM (335 - 369 us).
 constexpr int kStreamThreads = 256;
-constexpr int kStreamItems = 12;                          // nonzeros per thread and batch
+#ifndef CBG_STREAM_ITEMS
+#define CBG_STREAM_ITEMS 12
+#endif
+#ifndef CBG_STREAM_MINCTAS
+#define CBG_STREAM_MINCTAS 4
+#endif
+constexpr int kStreamItems = CBG_STREAM_ITEMS;            // nonzeros per thread and batch
 constexpr int kStreamT = kStreamThreads * kStreamItems;   // 3072 nonzeros per block
 constexpr int kStreamBuf = kStreamT + kStreamT / 2;       // + the overhang of the block's last row (36 KB)
 constexpr int kLongRow = 64;                              // rows longer than 64 g are reduced by a whole warp
@@ -219,10 +238,17 @@ __device__ __forceinline__ int ldg_stream_i32(const int32_t *p, uint64_t pol)
     asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.b32 %0, [%1], %2;" : "=r"(r) : "l"(p), "l"(pol));
     return r;
 }
-__device__ __forceinline__ double ldg_stream_f64(const double *p, uint64_t pol)
+
+// 8-byte asynchronous copy global -> shared (LDGSTS): no register holds the value while it is in flight
+__device__ __forceinline__ void cp_async8_hint(void *dst_smem, const void *src, uint64_t pol)
 {
-    double r;
-    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(r) : "l"(p), "l"(pol));
+    asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 8, %2;" ::"r"(smem_u32(dst_smem)), "l"(src), "l"(pol) : "memory");
+}
+// row pointers: volatile, so that the loads are issued where they are written (ahead of the phase that needs them)
+__device__ __forceinline__ int ldg_rowptr(const int32_t *p)
+{
+    int r;
+    asm volatile("ld.global.nc.b32 %0, [%1];" : "=r"(r) : "l"(p));
     return r;
 }
 
@@ -232,10 +258,21 @@ __device__ __forceinline__ double ldg_stream_f64(const double *p, uint64_t pol)
 #ifndef CBG_GATHER
 #define CBG_GATHER 1
 #endif
+#ifndef CBG_GATHER_VOLATILE
+#define CBG_GATHER_VOLATILE 1
+#endif
 __device__ __forceinline__ double gather_x(const double *p)
 {
 #if CBG_GATHER == 1
+#if CBG_GATHER_VOLATILE
+    // volatile: keeps the program order "all index / value loads, then all gathers, then the products" -- the
+    // compiler otherwise interleaves gather -> multiply -> store per item to save registers
+    double r;
+    asm volatile("ld.global.cg.f64 %0, [%1];" : "=d"(r) : "l"(p));
+    return r;
+#else
     return __ldcg(p);
+#endif
 #elif CBG_GATHER == 2
     double r;
     asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(r) : "l"(p));
@@ -245,7 +282,7 @@ __device__ __forceinline__ double gather_x(const double *p)
 #endif
 }
 
-__global__ void __launch_bounds__(kStreamThreads) spmv_stream_kernel(const SpmvArgs a)
+__global__ void __launch_bounds__(kStreamThreads, CBG_STREAM_MINCTAS) spmv_stream_kernel(const SpmvArgs a)
 {
     pdl_wait();
     pdl_launch_dependents();
@@ -266,34 +303,51 @@ __global__ void __launch_bounds__(kStreamThreads) spmv_stream_kernel(const SpmvA
         const int r0 = d.x, r1 = d.y, p0 = d.z, cnt = d.w - d.z;
         if (r0 >= r1) continue;
         if (cnt <= kStreamBuf) {
+            // row pointers of this thread's first row of phase 2: on their way while phase 1 runs
+            int rr = r0 + tid / g;
+            int pa0 = p0, pa1 = p0;
+            if (rr < r1) {
+                pa0 = ldg_rowptr(rp + rr);
+                pa1 = ldg_rowptr(rp + rr + 1);
+            }
             __syncthreads(); // the previous block's phase 2 has finished with prod[]
             for (int off = 0; off < cnt; off += kStreamT) {
+                // values: global -> shared memory without passing through registers (the registers go to the gathers)
+#pragma unroll
+                for (int i = 0; i < kStreamItems; ++i) {
+                    const int q = off + i * kStreamThreads + tid;
+                    if (q < cnt) cp_async8_hint(&prod[q], va + p0 + q, pol);
+                }
+                asm volatile("cp.async.commit_group;" ::: "memory");
                 int c[kStreamItems];
-                double v[kStreamItems];
 #pragma unroll
                 for (int i = 0; i < kStreamItems; ++i) {
                     const int q = off + i * kStreamThreads + tid;
                     c[i] = 0;
-                    v[i] = 0.0;
-                    if (q < cnt) {
-                        c[i] = ldg_stream_i32(ci + p0 + q, pol);
-                        v[i] = ldg_stream_f64(va + p0 + q, pol);
-                    }
+                    if (q < cnt) c[i] = ldg_stream_i32(ci + p0 + q, pol);
                 }
                 double xv[kStreamItems];
 #pragma unroll
                 for (int i = 0; i < kStreamItems; ++i) xv[i] = gather_x(x + c[i]);
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
 #pragma unroll
                 for (int i = 0; i < kStreamItems; ++i) {
                     const int q = off + i * kStreamThreads + tid;
-                    if (q < cnt) prod[q] = v[i] * xv[i];
+                    if (q < cnt) prod[q] *= xv[i]; // the thread that copied value q multiplies it: no barrier in between
                 }
             }
             __syncthreads();
             for (int rb = r0; rb < r1; rb += rows_per_pass) {
                 const int r = rb + tid / g;
                 const bool valid = r < r1;
-                const int a0 = valid ? rp[r] - p0 : 0, a1 = valid ? rp[r + 1] - p0 : 0;
+                const int a0 = pa0 - p0, a1 = pa1 - p0;
+                // the next pass's row pointers (an L2 round trip each) are fetched under this pass's reduction
+                rr = r + rows_per_pass;
+                pa0 = pa1 = p0;
+                if (rr < r1) {
+                    pa0 = ldg_rowptr(rp + rr);
+                    pa1 = ldg_rowptr(rp + rr + 1);
+                }
                 const double bv = (valid && a.mode == MODE_RESIDUAL) ? a.b[r] : 0.0;
                 const bool is_long = valid && (a1 - a0) > kLongRow * g;
                 double s = 0.0;
@@ -370,7 +424,10 @@ __global__ void __launch_bounds__(kStreamThreads) spmv_stream_kernel(const SpmvA
 // 587 / 621 / 795 us) nor smaller blocks at four CTAs per SM (634 us) moves the bound.
 constexpr int kTmaThreads = 256;                 // consumers
 constexpr int kTmaCta = kTmaThreads + 32;        // + the producer warp
-constexpr int kTmaItems = 8;                     // gathers in flight per thread and batch
+#ifndef CBG_TMA_ITEMS
+#define CBG_TMA_ITEMS 8
+#endif
+constexpr int kTmaItems = CBG_TMA_ITEMS;         // gathers in flight per thread and batch
 constexpr int kTmaT = kTmaThreads * kTmaItems;   // 2048 nonzeros per block
 constexpr int kTmaBuf = kTmaT + kTmaT / 2;       // + the overhang of the block's last row
 constexpr int kTmaMaxRows = kTmaBuf;             // rows of a staged block (rows may be as short as one entry)
