@@ -153,8 +153,12 @@ def full(rep, out_prefix, cmd, note):
 
 def source(rep, out_md, launch, top, cmd, note):
     """Hot spots of one captured launch: SASS instructions ranked by executed warp instructions."""
-    txt = subprocess.run(["ncu", "-i", rep, "--page", "source", "--csv", "--print-source", "sass"],
-                         capture_output=True, text=True).stdout
+    if rep.endswith(".csv"):  # the source page already exported on the GPU box (`ncu -i REP --page source --csv --print-source sass`)
+        with open(rep) as f:
+            txt = f.read()
+    else:
+        txt = subprocess.run(["ncu", "-i", rep, "--page", "source", "--csv", "--print-source", "sass"],
+                             capture_output=True, text=True).stdout
     rows = list(csv.reader(io.StringIO(txt)))
     starts = [i for i, r in enumerate(rows) if r and r[0] == "Kernel Name"]  # one section per captured launch
     if launch >= len(starts):
