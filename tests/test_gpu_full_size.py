@@ -219,10 +219,17 @@ def test_full_size_solve_matches_cached_oracle(full_solvers, case, fmt):
     assert r.rel_res_true == pytest.approx(true, rel=1e-6)
     if o["converged"]:
         assert true <= p.rel_tol * (1 + 1e-9) and o["rel_res_true_recomputed"] <= p.rel_tol * (1 + 1e-9)
-    assert true <= 10 * o["rel_res_true_recomputed"] and o["rel_res_true_recomputed"] <= 10 * true
+    # "within 10x of each other" (north_star), against the range of the oracle's own residuals: its base run and the same
+    # solve under other summation orders.  The range is a point for every case but the 16-bit solves that do not converge
+    # (int16 on the Jacobi- / block-Jacobi-preconditioned power-law matrix: the oracle's own residuals at the iteration
+    # bound run from 3 to 2e5, reading Q11 and DESIGN.md section 6.6)
+    ores = [o["rel_res_true_recomputed"]] + [d["rel_res_true"] for d in o.get("spread", {}).values()]
+    assert true <= 10 * max(ores) and min(ores) <= 10 * true
     if rule == "strict":
         assert abs(r.restarts - o["restarts"]) <= 1
-        assert abs(r.reorth_count - o["reorth_count"]) <= max(2, 0.02 * o["reorth_count"])
+        # l.7 fires on almost every step of these solves, so the two counts can only be compared after allowing for the
+        # steps one side did and the other did not (reading Q11: the step counts themselves agree to +-2 %)
+        assert abs(r.reorth_count - o["reorth_count"]) <= max(2, 0.02 * o["reorth_count"]) + abs(r.iters - o["iters"])
     # the first steps are before any decorrelation: the recurrence residuals agree to the format's roundoff (40 steps on
     # the stencils; 12 on the power-law matrix, whose quantised histories part within some tens of steps: reading Q11)
     c4 = case.startswith("C4")
