@@ -46,8 +46,8 @@ UNIT = "iters/s"
 PROFILE_EVERY = 2       # separate pass after the timed regions: CUDA-event brackets around the kernels of every 2nd Arnoldi step
 # Arnoldi steps per format in one step of the reference arm / cpu_baseline: sized so that `--steps 20 --warmup 5` of the
 # reference arm ends within a few minutes on the GPU box's host cores (an oracle step at basis size j streams about
-# 12 nnz + 100 j n bytes: C5 ~ 0.2 s at j <= 8, C2 ~ 0.03 s at j <= 60)
-REF_ITERS = {"C5": 8, "C2": 60, "C2small": 60, "C4": 20, "C1": 3000}
+# 12 nnz + 100 j n bytes: on 16 cores one such step of the reference arm takes ~ 7 s on C5, ~ 2 s on C2)
+REF_ITERS = {"C5": 24, "C2": 60, "C2small": 60, "C4": 20, "C1": 3000}
 PRECOND = "none"        # --precond: the paper's right preconditioners on both arms
 WORKLOADS = {"C5": {}, "C2": {}, "C1": {}, "C4": {}, "C2small": {"name": "C2", "grid": 32}}
 NOMINAL_HBM_GBS = 8000.0  # BASELINE.json north_star: "B200 peak (~8 TB/s)"
